@@ -1,0 +1,109 @@
+"""ctypes loader for the CPU oracle (oracle/bg_oracle.c).
+
+TEST INFRASTRUCTURE: only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this package.  It never imports
+the CUDA package and shares no code with it.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+import threading
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "liboracle_bg.so")
+_SRC = [os.path.join(_HERE, "bg_oracle.c"), os.path.join(_HERE, "bg_recursion.inc")]
+_LIB = None
+
+FP31, C128, C80 = 0, 1, 2
+P31 = (1 << 31) - 1
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2, FP contraction off so complex128 results are reproducible across hosts."""
+    if not force and os.path.exists(_SO) and all(
+            os.path.getmtime(_SO) >= os.path.getmtime(s) for s in _SRC):
+        return _SO
+    cmd = ["gcc", "-std=c11", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fPIC", "-shared",
+           "-Wall", "-Wextra", "-o", _SO, _SRC[0], "-lm"]
+    subprocess.run(cmd, check=True, cwd=_HERE)
+    return _SO
+
+
+def _lib():
+    global _LIB
+    if _LIB is None:
+        build()
+        lib = ctypes.CDLL(_SO)
+        vp, i64, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int
+        lib.oracle_bg_currents.argtypes = [ci, ci, ci, i64, vp, vp, vp, vp, vp]
+        lib.oracle_bg_currents.restype = ci
+        lib.oracle_bg_amplitudes.argtypes = [ci, ci, ci, i64, vp, vp, vp, vp]
+        lib.oracle_bg_amplitudes.restype = ci
+        lib.oracle_bg_modulus.restype = ctypes.c_uint32
+        _LIB = lib
+    return _LIB
+
+
+def _dtypes(field: int):
+    if field == FP31:
+        return np.uint32, np.uint32
+    if field == C128:
+        return np.complex128, np.complex128
+    if field == C80:
+        return np.complex128, np.clongdouble
+    raise ValueError("field must be FP31, C128 or C80")
+
+
+def amplitudes(field: int, momenta: np.ndarray, polarisations: np.ndarray,
+               want_currents: bool = False, want_status: bool = False, threads: int = 1):
+    """momenta, polarisations: [batch, n, d].  Returns out [batch] (and, on request,
+    currents [batch, m, m, d] and status [batch]).  threads > 1 splits the batch into
+    contiguous slices, one Python thread each (ctypes releases the GIL)."""
+    in_dt, out_dt = _dtypes(field)
+    mom = np.ascontiguousarray(momenta, dtype=in_dt)
+    pol = np.ascontiguousarray(polarisations, dtype=in_dt)
+    if mom.ndim != 3 or mom.shape != pol.shape:
+        raise ValueError("momenta and polarisations must both be [batch, n, d]")
+    batch, n, d = mom.shape
+    m = n - 1
+    out = np.zeros(batch, dtype=out_dt)
+    cur = np.zeros((batch, m, m, d), dtype=out_dt) if want_currents else None
+    status = np.zeros(batch, dtype=np.uint32)
+    lib = _lib()
+    rc = [0] * max(1, threads)
+
+    def run(t, b0, b1):
+        if b1 <= b0:
+            return
+        rc[t] = lib.oracle_bg_currents(
+            field, n, d, b1 - b0, mom[b0:b1].ctypes.data, pol[b0:b1].ctypes.data,
+            out[b0:b1].ctypes.data, None if cur is None else cur[b0:b1].ctypes.data,
+            status[b0:b1].ctypes.data)
+
+    if threads <= 1 or batch < 2 * threads:
+        rc[0] = lib.oracle_bg_currents(
+            field, n, d, batch, mom.ctypes.data, pol.ctypes.data, out.ctypes.data,
+            None if cur is None else cur.ctypes.data, status.ctypes.data)
+    else:
+        bounds = [batch * t // threads for t in range(threads + 1)]
+        ts = [threading.Thread(target=run, args=(t, bounds[t], bounds[t + 1])) for t in range(threads)]
+        for t in ts:
+            t.start()
+        for t in ts:
+            t.join()
+    if any(r != 0 for r in rc):
+        raise ValueError("oracle rejected the arguments (need 4<=n<=16, 4<=d<=16)")
+    res = [out]
+    if want_currents:
+        res.append(cur)
+    if want_status:
+        res.append(status)
+    return res[0] if len(res) == 1 else tuple(res)
+
+
+def modulus() -> int:
+    return int(_lib().oracle_bg_modulus())

@@ -1,0 +1,318 @@
+"""Seeded synthetic kinematics for the Berends-Giele hot path.
+
+This module is the ONE piece shared by the CPU oracle (``oracle/``) and the CUDA
+path (``csrc/``): it only *prepares inputs* (on-shell, momentum-conserving momenta
+and transverse polarisation vectors).  It contains none of the method's arithmetic
+(no currents, no vertices, no recursion) and imports neither side.
+
+It stands in for the paper's host-side phase-space / state preparation, which
+uses ``lips``/``syngular`` (§3) and is not available
+here.  The recipe is the one BASELINE.json:configs states, made concrete in
+SURVEY.md §8(d) and DESIGN.md §"Input recipe":
+
+* every random number is a pure function of (seed, global point index, attempt,
+  draw counter) through SplitMix64, so any slice ``[start, start+batch)`` of a
+  workload can be generated independently (used for multi-GPU sharding);
+* massless vectors come from light-cone data: p- = (sum p_perp^2) / (2 p+),
+  Cartesian p^0 = p+ + p-/2, p^1 = p+ - p-/2, p^{2..d-1} = p_perp, metric
+  diag(+,-,...,-);
+* p_1..p_{n-2} free, K = -(p_1+..+p_{n-2}), q random massless,
+  p_{n-1} = alpha q with alpha = K^2/(2 K.q), p_n = K - p_{n-1};
+* generic polarisations eps_i = v_i - (v_i.p_i)/(r_i.p_i) r_i  (transverse,
+  unnormalised), or, for d = 4 complex, spinor-helicity states eps_-/eps_+ built
+  on the reference momentum r_i (used for the Parke-Taylor pin).
+"""
+from __future__ import annotations
+
+import numpy as np
+
+P31 = (1 << 31) - 1  # the prime of BASELINE.json:configs, p = 2^31 - 1
+
+_U64 = np.uint64
+_GOLDEN = _U64(0x9E3779B97F4A7C15)
+_M1 = _U64(0xBF58476D1CE4E5B9)
+_M2 = _U64(0x94D049BB133111EB)
+
+
+def _mix64(z: np.ndarray) -> np.ndarray:
+    """SplitMix64 output function (finaliser) on uint64 arrays, wrapping."""
+    with np.errstate(over="ignore"):
+        z = (z ^ (z >> _U64(30))) * _M1
+        z = (z ^ (z >> _U64(27))) * _M2
+        return z ^ (z >> _U64(31))
+
+
+class _Stream:
+    """Counter-based stream: draw c of point b, attempt a is
+    mix64(key(seed, b, a) + (c+1)*GOLDEN).  Vectorised over points."""
+
+    def __init__(self, seed: int, index: np.ndarray, attempt: np.ndarray):
+        with np.errstate(over="ignore"):
+            k = _mix64(np.full(index.shape, seed, dtype=_U64) + _GOLDEN)
+            k = _mix64(k ^ (index.astype(_U64) * _M1 + _GOLDEN))
+            k = _mix64(k ^ (attempt.astype(_U64) * _M2 + _GOLDEN))
+        self.key = k
+        self.counter = 0
+
+    def u64(self, count: int) -> np.ndarray:
+        """next `count` draws for every point -> uint64 [points, count]"""
+        c = np.arange(self.counter + 1, self.counter + count + 1, dtype=_U64)
+        self.counter += count
+        with np.errstate(over="ignore"):
+            return _mix64(self.key[:, None] + c[None, :] * _GOLDEN)
+
+
+# ---------------------------------------------------------------------------
+# F_p helpers (input preparation only)
+# ---------------------------------------------------------------------------
+_P = _U64(P31)
+
+
+def _fp_mul(a, b):
+    return (a * b) % _P  # operands < 2^31, product < 2^62 fits uint64
+
+
+def _fp_sub(a, b):
+    return (a + _P - b) % _P
+
+
+def _fp_pow(a, e: int):
+    r = np.ones_like(a)
+    base = a.copy()
+    while e:
+        if e & 1:
+            r = _fp_mul(r, base)
+        base = _fp_mul(base, base)
+        e >>= 1
+    return r
+
+
+def _fp_inv(a):
+    return _fp_pow(a, P31 - 2)
+
+
+def _fp_dot(x, y):
+    """Minkowski product, metric diag(+,-,...,-), last axis = component."""
+    t = _fp_mul(x, y)
+    time = t[..., 0]
+    space = t[..., 1:].sum(axis=-1) % _P
+    return _fp_sub(time, space)
+
+
+_INV2 = _U64((P31 + 1) // 2)
+
+
+def _fp_massless(plus, perp):
+    """light-cone -> Cartesian massless vector. plus [..], perp [.., d-2] -> [.., d]"""
+    perp2 = _fp_mul(perp, perp).sum(axis=-1) % _P
+    minus = _fp_mul(perp2, _fp_inv(_fp_mul(_U64(2), plus)))
+    half = _fp_mul(minus, _INV2)
+    p0 = (plus + half) % _P
+    p1 = _fp_sub(plus, half)
+    return np.concatenate([p0[..., None], p1[..., None], perp], axis=-1)
+
+
+def _fp_generate(n: int, d: int, seed: int, index: np.ndarray, attempt: np.ndarray):
+    """One attempt for every listed point. Returns mom, pol (uint64) and ok mask."""
+    st = _Stream(seed, index, attempt)
+    nb = index.shape[0]
+    dt = d - 2
+    mom = np.zeros((nb, n, d), dtype=_U64)
+    raw = st.u64((n - 2) * (d - 1)).reshape(nb, n - 2, d - 1)
+    plus = _U64(1) + raw[:, :, 0] % _U64(P31 - 1)       # uniform in [1,p)
+    perp = _U64(1) + raw[:, :, 1:] % _U64(P31 - 1)      # uniform in [1,p)
+    mom[:, : n - 2] = _fp_massless(plus, perp)
+    raw = st.u64(d - 1)
+    q = _fp_massless(_U64(1) + raw[:, 0] % _U64(P31 - 1),
+                     _U64(1) + raw[:, 1:] % _U64(P31 - 1))
+    ksum = mom[:, : n - 2].sum(axis=1) % _P
+    K = (_P - ksum) % _P
+    K2 = _fp_dot(K, K)
+    Kq = _fp_dot(K, q)
+    ok = Kq != 0
+    alpha = _fp_mul(K2, _fp_inv(_fp_mul(_U64(2), Kq)))
+    mom[:, n - 2] = _fp_mul(alpha[:, None], q)
+    mom[:, n - 1] = _fp_sub(K, mom[:, n - 2])
+    # polarisations: per leg v (d draws, uniform in F_p) then r (p+, p_perp in [1,p))
+    raw = st.u64(n * (2 * d - 1)).reshape(nb, n, 2 * d - 1)
+    v = raw[:, :, :d] % _P
+    r = _fp_massless(_U64(1) + raw[:, :, d] % _U64(P31 - 1),
+                     _U64(1) + raw[:, :, d + 1:] % _U64(P31 - 1))
+    vp = _fp_dot(v, mom)
+    rp = _fp_dot(r, mom)
+    ok &= (rp != 0).all(axis=1)
+    coef = _fp_mul(vp, _fp_inv(rp))
+    pol = _fp_sub(v, _fp_mul(coef[..., None], r))
+    # reject points with a vanishing proper invariant P_{i,j}^2, 1<=i<j<=n-1, (i,j)!=(1,n-1)
+    m = n - 1
+    prefix = np.zeros((nb, m + 1, d), dtype=_U64)
+    for j in range(1, m + 1):
+        prefix[:, j] = (prefix[:, j - 1] + mom[:, j - 1]) % _P
+    for i in range(1, m + 1):
+        for j in range(i + 1, m + 1):
+            if i == 1 and j == m:
+                continue
+            Pij = _fp_sub(prefix[:, j], prefix[:, i - 1])
+            ok &= _fp_dot(Pij, Pij) != 0
+    del dt
+    return mom, pol, ok
+
+
+def make_fp_inputs(n: int, d: int, batch: int, seed: int = 0, start: int = 0):
+    """F_p (p = 2^31-1) workload slice [start, start+batch).
+
+    Returns (momenta, polarisations, info): uint32 arrays [batch, n, d] of canonical
+    residues, all momenta outgoing; info = {"redraws": number of rejected attempts}.
+    Points with K.q = 0, r_i.p_i = 0 or a vanishing proper P_{i,j}^2 are redrawn
+    deterministically with attempt+1."""
+    if n < 4 or d < 3:
+        raise ValueError("need n >= 4 and d >= 3")
+    index = np.arange(start, start + batch, dtype=_U64)
+    mom = np.zeros((batch, n, d), dtype=np.uint32)
+    pol = np.zeros((batch, n, d), dtype=np.uint32)
+    todo = np.arange(batch)
+    attempt = np.zeros(batch, dtype=_U64)
+    redraws = 0
+    chunk = 1 << 16
+    while todo.size:
+        nxt = []
+        for c0 in range(0, todo.size, chunk):
+            sel = todo[c0:c0 + chunk]
+            m_, p_, ok = _fp_generate(n, d, seed, index[sel], attempt[sel])
+            good = sel[ok]
+            mom[good] = m_[ok].astype(np.uint32)
+            pol[good] = p_[ok].astype(np.uint32)
+            nxt.append(sel[~ok])
+        todo = np.concatenate(nxt) if nxt else np.zeros(0, dtype=np.int64)
+        attempt[todo] += _U64(1)
+        redraws += int(todo.size)
+    return mom, pol, {"redraws": redraws}
+
+
+# ---------------------------------------------------------------------------
+# complex128
+# ---------------------------------------------------------------------------
+def _c_uniform(raw: np.ndarray) -> np.ndarray:
+    """uint64 [..., 2k] -> complex [..., k], re and im each (u>>11)*2^-52 - 1 in [-1,1)."""
+    f = (raw >> _U64(11)).astype(np.float64) * (2.0 ** -52) - 1.0
+    return f[..., 0::2] + 1j * f[..., 1::2]
+
+
+def _c_dot(x, y):
+    t = x * y
+    return t[..., 0] - t[..., 1:].sum(axis=-1)
+
+
+def _c_massless(plus, perp):
+    minus = (perp * perp).sum(axis=-1) / (2.0 * plus)
+    p0 = plus + 0.5 * minus
+    p1 = plus - 0.5 * minus
+    return np.concatenate([p0[..., None], p1[..., None], perp], axis=-1)
+
+
+def spinors(p: np.ndarray):
+    """Holomorphic/antiholomorphic spinors of a (complex) massless 4-vector.
+
+    M = [[p0+p3, p1-i p2],[p1+i p2, p0-p3]] = lam lamt^T with lam = (M00, M10),
+    lamt = (1, M01/M00).  Returns (lam [...,2], lamt [...,2])."""
+    M00 = p[..., 0] + p[..., 3]
+    M01 = p[..., 1] - 1j * p[..., 2]
+    M10 = p[..., 1] + 1j * p[..., 2]
+    lam = np.stack([M00, M10], axis=-1)
+    lamt = np.stack([np.ones_like(M00), M01 / M00], axis=-1)
+    return lam, lamt
+
+
+def spinor_bracket(a: np.ndarray, b: np.ndarray) -> np.ndarray:
+    """<ab> (or [ab] when fed lamt's) = a0 b1 - a1 b0."""
+    return a[..., 0] * b[..., 1] - a[..., 1] * b[..., 0]
+
+
+def _bispinor_to_vector(N00, N01, N10, N11):
+    return np.stack([(N00 + N11) / 2, (N01 + N10) / 2, (N10 - N01) / 2j, (N00 - N11) / 2], axis=-1)
+
+
+def helicity_polarisation(k: np.ndarray, r: np.ndarray, hel: int) -> np.ndarray:
+    """sqrt-free spinor-helicity states in d=4 (weights 1/2 * 2 as in Eq.(11)):
+       eps_-(k;r) = vec(lam_k lamt_r^T) / [r k],  eps_+(k;r) = 2 vec(lam_r lamt_k^T) / <r k>.
+    eps_+.eps_- = -1, eps_h.eps_h = 0, eps.k = 0."""
+    lk, ltk = spinors(k)
+    lr, ltr = spinors(r)
+    if hel < 0:
+        a, b, den, w = lk, ltr, spinor_bracket(ltr, ltk), 1.0
+    else:
+        a, b, den, w = lr, ltk, spinor_bracket(lr, lk), 2.0
+    vec = _bispinor_to_vector(a[..., 0] * b[..., 0], a[..., 0] * b[..., 1],
+                              a[..., 1] * b[..., 0], a[..., 1] * b[..., 1])
+    return w * vec / den[..., None]
+
+
+def make_complex_inputs(n: int, d: int, batch: int, seed: int = 0, start: int = 0,
+                        helicities=None):
+    """complex128 workload slice.  Momenta: the light-cone/alpha construction with
+    complex components (re, im uniform in [-1,1)).  Polarisations: generic transverse
+    vectors (helicities=None) or, for d == 4, spinor-helicity states with the given
+    signs (e.g. (-1,-1,+1,+1,+1,+1) for config 1) on random reference momenta r_i.
+    No rejection.  Returns (mom, pol, info); info carries the
+    reference momenta so tests can rebuild the spinors."""
+    if n < 4 or d < 3:
+        raise ValueError("need n >= 4 and d >= 3")
+    if helicities is not None and (d != 4 or len(helicities) != n):
+        raise ValueError("helicity states need d == 4 and one sign per leg")
+    mom = np.zeros((batch, n, d), dtype=np.complex128)
+    pol = np.zeros((batch, n, d), dtype=np.complex128)
+    ref = np.zeros((batch, n, d), dtype=np.complex128)
+    chunk = 1 << 16
+    for c0 in range(0, batch, chunk):
+        nb = min(chunk, batch - c0)
+        index = np.arange(start + c0, start + c0 + nb, dtype=_U64)
+        st = _Stream(seed, index, np.zeros(nb, dtype=_U64))
+        raw = _c_uniform(st.u64(2 * (n - 2) * (d - 1))).reshape(nb, n - 2, d - 1)
+        m_ = np.zeros((nb, n, d), dtype=np.complex128)
+        m_[:, : n - 2] = _c_massless(raw[:, :, 0], raw[:, :, 1:])
+        raw = _c_uniform(st.u64(2 * (d - 1)))
+        q = _c_massless(raw[:, 0], raw[:, 1:])
+        K = -m_[:, : n - 2].sum(axis=1)
+        alpha = _c_dot(K, K) / (2.0 * _c_dot(K, q))
+        m_[:, n - 2] = alpha[:, None] * q
+        m_[:, n - 1] = K - m_[:, n - 2]
+        raw = _c_uniform(st.u64(2 * n * (2 * d - 1))).reshape(nb, n, 2 * d - 1)
+        v = raw[:, :, :d]
+        r = _c_massless(raw[:, :, d], raw[:, :, d + 1:])
+        if helicities is None:
+            coef = _c_dot(v, m_) / _c_dot(r, m_)
+            p_ = v - coef[..., None] * r
+        else:
+            p_ = np.zeros((nb, n, d), dtype=np.complex128)
+            for i, h in enumerate(helicities):
+                p_[:, i] = helicity_polarisation(m_[:, i], r[:, i], int(h))
+        mom[c0:c0 + nb], pol[c0:c0 + nb], ref[c0:c0 + nb] = m_, p_, r
+    return mom, pol, {"redraws": 0, "reference": ref}
+
+
+# ---------------------------------------------------------------------------
+# the five workloads of BASELINE.json:configs
+# ---------------------------------------------------------------------------
+CONFIGS = {
+    "cfg0": dict(n=4, d=4, field="fp31", batch=1 << 10, helicities=None),
+    "cfg1": dict(n=6, d=4, field="c128", batch=1 << 20, helicities=(-1, -1, 1, 1, 1, 1)),
+    "cfg2": dict(n=8, d=6, field="fp31", batch=1 << 20, helicities=None),
+    "cfg3": dict(n=10, d=8, field="fp31", batch=1 << 18, helicities=None),
+    "cfg4a": dict(n=12, d=6, field="fp31", batch=1 << 16, helicities=None),
+    "cfg4b": dict(n=12, d=6, field="c128", batch=1 << 16, helicities=None),
+}
+
+
+def make_inputs(field: str, n: int, d: int, batch: int, seed: int = 0, start: int = 0,
+                helicities=None):
+    if field == "fp31":
+        return make_fp_inputs(n, d, batch, seed, start)
+    if field == "c128":
+        return make_complex_inputs(n, d, batch, seed, start, helicities)
+    raise ValueError(f"unknown field {field!r}")
+
+
+def make_config(name: str, batch: int | None = None, seed: int = 0, start: int = 0):
+    c = CONFIGS[name]
+    return make_inputs(c["field"], c["n"], c["d"], c["batch"] if batch is None else batch,
+                       seed, start, c["helicities"])
