@@ -1,0 +1,158 @@
+/* bg.h -- C ABI of libbg_b200: batched colour-ordered n-gluon tree amplitudes by
+ * Berends-Giele recursion in d space-time dimensions, over F_p (p = 2^31-1) and
+ * complex128, on one NVIDIA B200 (sm_100a).
+ *
+ * Reference: arXiv:2502.07060 ("Accelerating Berends-Giele recursion for gluons in
+ * arbitrary dimensions over finite fields"); citations are PAPER.md:<line>.
+ *
+ * What one call computes, per phase-space point b (points are independent; the paper
+ * parallelises "strictly along the event dimension"):
+ *
+ *     P_{i,j} = sum_{l=i..j} k_l                                   Eq.(7)
+ *     J(i..i) = eps_i
+ *     J(i..j) = 1/P_{i,j}^2 [ sum_k V3(P_{i,k},P_{k+1,j}) J(i..k) J(k+1..j)
+ *                           + sum_{k<l} V4 J(i..k) J(k+1..l) J(l+1..j) ]   Eq.(6)
+ *     out[b]  = eps_n . N(1..n-1)     N = the bracket above for the (n-1)-gluon current,
+ *                                     no propagator on it
+ *
+ * with V3, V4 of Eq.(7), metric g = diag(+,-,...,-) and
+ * the factors of i cancelled: (-i) of Eq.(6) times i of Eq.(7) = 1, so everything stays in
+ * F_p; the physical colour-ordered amplitude is i * out (readings R1-R5).
+ * The momenta and polarisation states are prepared by the caller on the host, exactly as
+ * in the paper.  Every step above runs inside hand-written sm_100a kernels;
+ * there is no CPU fallback and no other backend.
+ *
+ * Conventions common to all entry points
+ *   scalars   BG_FIELD_FP31: uint32_t residues; values >= p are reduced mod p on load;
+ *             results are canonical, in [0,p).
+ *             BG_FIELD_C128: double[2] = (re, im), interleaved.
+ *   layout    momenta, polarisations: [batch][n][d] scalars, point-major, contravariant
+ *             components, all momenta outgoing (sum_l k_l = 0 is the caller's job; the
+ *             library evaluates the map above for whatever it is given, reading R4).
+ *             out: [batch] scalars.
+ *   limits    4 <= n <= 16, 4 <= d <= 16 (the paper validates d = 4..10).
+ *   memory    the caller owns every buffer; DEVICE pointers unless the name says host.
+ *             Device pointers must be 16-byte aligned; out must not alias the inputs.
+ *             The library allocates no device memory and keeps no per-call state.
+ *   stream    launches are asynchronous on `stream`; nothing synchronises.
+ *   errors    return value: BG_OK or a negative bg_status_t; nothing is thrown, nothing
+ *             aborts.  Arguments are checked on the host before any launch.  batch == 0 is
+ *             a no-op returning BG_OK.
+ *   1/0       inv(0) := 0 in both fields (what Fermat's a^(p-2) gives); a point where some
+ *             proper P_{i,j}^2 vanishes gets status bit0 set (reading R6).
+ */
+#ifndef BG_B200_H
+#define BG_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* cudaStream_t without dragging cuda_runtime.h into C callers */
+#ifndef __DRIVER_TYPES_H__
+typedef struct CUstream_st* cudaStream_t;
+#endif
+
+typedef enum { BG_FIELD_FP31 = 0, BG_FIELD_C128 = 1 } bg_field_t;
+
+typedef enum {
+    BG_OK = 0,
+    BG_ERR_ARG = -1,          /* bad n, d, batch, field, null or misaligned pointer */
+    BG_ERR_UNSUPPORTED = -2,  /* (field, n, d) needs more shared memory per point than an SM has */
+    BG_ERR_CUDA = -3          /* a CUDA runtime call or launch failed */
+} bg_status_t;
+
+/* ---- the hot path (SURVEY.md §8(a) rows a0-a6 in ONE kernel launch) ------------------- */
+
+/* Amplitudes for `batch` points.  Device pointers.  Eq.(6)/(7). */
+int bg_amplitudes(int field, int n, int d, int64_t batch,
+                  const void* momenta, const void* polarisations, void* out,
+                  cudaStream_t stream);
+
+/* Same, plus a per-point status word: status[b] bit0 = some proper P_{i,j}^2 == 0
+ * (its propagator was taken as 0).  status: device, [batch] uint32, or NULL. */
+int bg_amplitudes_status(int field, int n, int d, int64_t batch,
+                         const void* momenta, const void* polarisations, void* out,
+                         uint32_t* status, cudaStream_t stream);
+
+/* Same map, but also returns every off-shell current (Eq.(6) by-products):
+ * currents: device, [batch][m][m][d] scalars, m = n-1; entry (i-1, j-1), i <= j, holds
+ * J(i..j) (the top one, J(1..m), WITHOUT propagator); entries with i > j are not written.
+ * currents may be NULL. */
+int bg_currents(int field, int n, int d, int64_t batch,
+                const void* momenta, const void* polarisations, void* out,
+                void* currents, uint32_t* status, cudaStream_t stream);
+
+/* End-to-end variant with HOST buffers (pinned memory recommended): copies the inputs to
+ * the device in chunks, runs the kernel and copies the results back, overlapping the three
+ * on internal streams; returns after everything has completed.  `workspace` is DEVICE
+ * scratch owned by the caller, `workspace_bytes` >= bg_host_workspace_bytes(...) for at
+ * least one chunk of 1024 points; more workspace = larger chunks. */
+int bg_amplitudes_host(int field, int n, int d, int64_t batch,
+                       const void* host_momenta, const void* host_polarisations,
+                       void* host_out, uint32_t* host_status,
+                       void* workspace, size_t workspace_bytes);
+size_t bg_host_workspace_bytes(int field, int n, int d, int64_t chunk_points);
+
+/* ---- introspection --------------------------------------------------------------------- */
+
+uint32_t bg_modulus(void);             /* 2147483647 */
+const char* bg_status_string(int status);
+const char* bg_version(void);
+
+/* Algorithmic operation counts per amplitude for the literal Eq.(6) evaluation (M_ref of
+ * SURVEY.md §8(d)), by formula; and the counts the shipped kernel executes. */
+typedef struct {
+    int64_t currents;        /* n(n-1)/2 */
+    int64_t propagators;     /* R = (n-1)(n-2)/2 - 1 */
+    int64_t splits3;         /* C(n,3) */
+    int64_t splits4;         /* C(n,4) */
+    int64_t mul_v3;          /* 6 d C(n,3) */
+    int64_t mul_v4;          /* 6 d C(n,4) */
+    int64_t mul_other;       /* d R + 3(R-1) + d R + d */
+    int64_t mul_ref;         /* M_ref = the three above */
+    int64_t mul_factored;    /* field multiplications the kernel's factored form performs */
+    int64_t bytes_in;        /* 2 n d w */
+    int64_t bytes_out;       /* w */
+} bg_opcount_t;
+int bg_op_count(int field, int n, int d, bg_opcount_t* out);
+
+/* Launch configuration the library would use for (field, n, d). */
+typedef struct {
+    int specialised;         /* 1: (n, d) compiled in; 0: runtime-n instance */
+    int threads_per_block;
+    int points_per_block;
+    int smem_bytes_per_block;
+    int smem_bytes_per_point;
+    int blocks_per_sm;       /* limited by shared memory */
+    int regs_per_thread;
+} bg_kernel_info_t;
+int bg_kernel_info(int field, int n, int d, bg_kernel_info_t* out);
+
+/* ---- measurement support ---------------------------------------------------------------- */
+
+/* Register-resident issue-rate microbenchmarks (csrc/bg_peaks.cu): launches one kernel of
+ * `blocks` x `threads` threads, each executing *ops_per_thread operations of the given
+ * kind.  The caller times the launch with CUDA events.  sink: device scratch of at least
+ * blocks*threads uint32 (never actually written). */
+typedef enum {
+    BG_PEAK_IMAD_WIDE = 0,   /* IMAD.WIDE.U32 (32x32+64 -> 64) */
+    BG_PEAK_IMAD = 1,        /* IMAD (32x32+32 -> 32) */
+    BG_PEAK_ALU = 2,         /* LOP3 / IADD3 */
+    BG_PEAK_MIX = 3,         /* IMAD.WIDE and ALU alternating (counts both) */
+    BG_PEAK_MODMUL = 4,      /* canonical Mersenne-31 modular multiplication: R_mm */
+    BG_PEAK_DFMA = 5,        /* FP64 fused multiply-add: R_dfma */
+    BG_PEAK_LDS32 = 6,       /* shared-memory loads, 4/8/16 bytes per lane */
+    BG_PEAK_LDS64 = 7,
+    BG_PEAK_LDS128 = 8
+} bg_peak_kind_t;
+int bg_peak_probe(int kind, int iters, int blocks, int threads, uint32_t* sink,
+                  int64_t* ops_per_thread, cudaStream_t stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BG_B200_H */

@@ -1,0 +1,236 @@
+"""Thin ctypes binding of libbg_b200.so (include/bg.h) -- argument marshalling only.
+
+Every step of the Berends-Giele path runs inside the CUDA kernels of the library;
+PyTorch is used for device memory and streams, nothing else.  There is no CPU
+fallback: if the library is missing or no CUDA device is present, calls raise.
+The low-level functions carry the C names (bg_amplitudes, bg_currents, ...); the
+`amplitudes()` / `currents()` helpers below only infer (field, n, d, batch) from
+tensor shapes and allocate the output.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+FIELD_FP31, FIELD_C128 = 0, 1
+BG_OK, BG_ERR_ARG, BG_ERR_UNSUPPORTED, BG_ERR_CUDA = 0, -1, -2, -3
+PEAK_KINDS = {"imad_wide": 0, "imad": 1, "alu": 2, "mix": 3, "modmul": 4, "dfma": 5,
+              "lds32": 6, "lds64": 7, "lds128": 8}
+P31 = (1 << 31) - 1
+
+EXPORTS = ["bg_amplitudes", "bg_amplitudes_status", "bg_currents", "bg_amplitudes_host",
+           "bg_host_workspace_bytes", "bg_modulus", "bg_status_string", "bg_version",
+           "bg_op_count", "bg_kernel_info", "bg_peak_probe"]
+
+
+class BgError(RuntimeError):
+    pass
+
+
+class OpCount(ctypes.Structure):
+    _fields_ = [(k, ctypes.c_int64) for k in
+                ("currents", "propagators", "splits3", "splits4", "mul_v3", "mul_v4", "mul_other",
+                 "mul_ref", "mul_factored", "bytes_in", "bytes_out")]
+
+
+class KernelInfo(ctypes.Structure):
+    _fields_ = [(k, ctypes.c_int) for k in
+                ("specialised", "threads_per_block", "points_per_block", "smem_bytes_per_block",
+                 "smem_bytes_per_point", "blocks_per_sm", "regs_per_thread")]
+
+
+_LIB = None
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def load(rebuild_if_stale: bool = False):
+    """dlopen the in-tree library.  Fails loudly if it is not there."""
+    global _LIB
+    if _LIB is not None:
+        return _LIB
+    if rebuild_if_stale:
+        _build.build()
+    if not os.path.exists(_build.LIB):
+        raise BgError(f"{_build.LIB} not built: run `python -m paper_2502_07060_b200.build` "
+                      "(there is no CPU fallback)")
+    lib = ctypes.CDLL(_build.LIB)
+    vp, i64, ci, sz = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_size_t
+    lib.bg_amplitudes.argtypes = [ci, ci, ci, i64, vp, vp, vp, vp]
+    lib.bg_amplitudes_status.argtypes = [ci, ci, ci, i64, vp, vp, vp, vp, vp]
+    lib.bg_currents.argtypes = [ci, ci, ci, i64, vp, vp, vp, vp, vp, vp]
+    lib.bg_amplitudes_host.argtypes = [ci, ci, ci, i64, vp, vp, vp, vp, vp, sz]
+    lib.bg_host_workspace_bytes.argtypes = [ci, ci, ci, i64]
+    lib.bg_host_workspace_bytes.restype = sz
+    lib.bg_modulus.restype = ctypes.c_uint32
+    lib.bg_status_string.argtypes = [ci]
+    lib.bg_status_string.restype = ctypes.c_char_p
+    lib.bg_version.restype = ctypes.c_char_p
+    lib.bg_op_count.argtypes = [ci, ci, ci, ctypes.POINTER(OpCount)]
+    lib.bg_kernel_info.argtypes = [ci, ci, ci, ctypes.POINTER(KernelInfo)]
+    lib.bg_peak_probe.argtypes = [ci, ci, ci, ci, vp, ctypes.POINTER(i64), vp]
+    for name in ("bg_amplitudes", "bg_amplitudes_status", "bg_currents", "bg_amplitudes_host",
+                 "bg_op_count", "bg_kernel_info", "bg_peak_probe"):
+        getattr(lib, name).restype = ci
+    _LIB = lib
+    return lib
+
+
+def _check(rc: int):
+    if rc != BG_OK:
+        raise BgError(f"libbg_b200: {load().bg_status_string(rc).decode()} ({rc})")
+
+
+# ------------------------------------------------------------- C names, raw pointers
+def bg_amplitudes(field, n, d, batch, momenta_ptr, polarisations_ptr, out_ptr, stream_ptr=0):
+    return load().bg_amplitudes(field, n, d, batch, momenta_ptr, polarisations_ptr, out_ptr, stream_ptr)
+
+
+def bg_amplitudes_status(field, n, d, batch, momenta_ptr, polarisations_ptr, out_ptr, status_ptr,
+                         stream_ptr=0):
+    return load().bg_amplitudes_status(field, n, d, batch, momenta_ptr, polarisations_ptr, out_ptr,
+                                       status_ptr, stream_ptr)
+
+
+def bg_currents(field, n, d, batch, momenta_ptr, polarisations_ptr, out_ptr, currents_ptr, status_ptr,
+                stream_ptr=0):
+    return load().bg_currents(field, n, d, batch, momenta_ptr, polarisations_ptr, out_ptr,
+                              currents_ptr, status_ptr, stream_ptr)
+
+
+def bg_amplitudes_host(field, n, d, batch, host_mom_ptr, host_pol_ptr, host_out_ptr, host_status_ptr,
+                       workspace_ptr, workspace_bytes):
+    return load().bg_amplitudes_host(field, n, d, batch, host_mom_ptr, host_pol_ptr, host_out_ptr,
+                                     host_status_ptr, workspace_ptr, workspace_bytes)
+
+
+def bg_host_workspace_bytes(field, n, d, chunk_points):
+    return int(load().bg_host_workspace_bytes(field, n, d, chunk_points))
+
+
+def bg_modulus():
+    return int(load().bg_modulus())
+
+
+def bg_version():
+    return load().bg_version().decode()
+
+
+def bg_status_string(rc):
+    return load().bg_status_string(rc).decode()
+
+
+def bg_op_count(field, n, d) -> dict:
+    oc = OpCount()
+    _check(load().bg_op_count(field, n, d, ctypes.byref(oc)))
+    return {k: int(getattr(oc, k)) for k, _ in OpCount._fields_}
+
+
+def bg_kernel_info(field, n, d) -> dict:
+    ki = KernelInfo()
+    _check(load().bg_kernel_info(field, n, d, ctypes.byref(ki)))
+    return {k: int(getattr(ki, k)) for k, _ in KernelInfo._fields_}
+
+
+def bg_peak_probe(kind, iters, blocks, threads, sink_ptr, stream_ptr=0) -> int:
+    ops = ctypes.c_int64(0)
+    _check(load().bg_peak_probe(PEAK_KINDS[kind] if isinstance(kind, str) else kind, iters, blocks,
+                                threads, sink_ptr, ctypes.byref(ops), stream_ptr))
+    return int(ops.value)
+
+
+# ------------------------------------------------------------- tensor helpers
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise BgError("no CUDA device: the Berends-Giele path has no CPU fallback")
+    return torch
+
+
+def field_of(t) -> int:
+    import torch
+    if t.dtype in (torch.int32, torch.uint32):
+        return FIELD_FP31
+    if t.dtype == torch.complex128:
+        return FIELD_C128
+    raise BgError(f"unsupported dtype {t.dtype}: use uint32/int32 (F_p) or complex128")
+
+
+def to_device(arr: np.ndarray, device="cuda"):
+    """numpy [batch,n,d] uint32 / complex128 -> device tensor (F_p stored as int32 bits)"""
+    torch = _torch()
+    if arr.dtype == np.uint32:
+        return torch.from_numpy(arr.view(np.int32)).to(device)
+    return torch.from_numpy(np.ascontiguousarray(arr)).to(device)
+
+
+def to_numpy(t) -> np.ndarray:
+    import torch
+    a = t.detach().cpu().numpy()
+    return a.view(np.uint32) if t.dtype == torch.int32 else a
+
+
+def _prep(momenta, polarisations):
+    torch = _torch()
+    if momenta.shape != polarisations.shape or momenta.dim() != 3:
+        raise BgError("momenta and polarisations must both be [batch, n, d]")
+    if momenta.dtype != polarisations.dtype or not momenta.is_cuda or not polarisations.is_cuda:
+        raise BgError("momenta and polarisations must be CUDA tensors of the same dtype")
+    if not (momenta.is_contiguous() and polarisations.is_contiguous()):
+        raise BgError("inputs must be contiguous")
+    batch, n, d = momenta.shape
+    return torch, field_of(momenta), int(batch), int(n), int(d)
+
+
+def amplitudes(momenta, polarisations, out=None, status=None, stream=None):
+    """out[b] = eps_n . N(1..n-1) for every point of the batch (one kernel launch)."""
+    torch, field, batch, n, d = _prep(momenta, polarisations)
+    if out is None:
+        out = torch.empty(batch, dtype=momenta.dtype, device=momenta.device)
+    s = (stream or torch.cuda.current_stream(momenta.device)).cuda_stream
+    with torch.cuda.device(momenta.device):
+        if status is None:
+            _check(bg_amplitudes(field, n, d, batch, momenta.data_ptr(), polarisations.data_ptr(),
+                                 out.data_ptr(), s))
+        else:
+            _check(bg_amplitudes_status(field, n, d, batch, momenta.data_ptr(), polarisations.data_ptr(),
+                                        out.data_ptr(), status.data_ptr(), s))
+    return out
+
+
+def currents(momenta, polarisations, stream=None):
+    """returns (out [batch], currents [batch, m, m, d], status [batch] int32)"""
+    torch, field, batch, n, d = _prep(momenta, polarisations)
+    m = n - 1
+    out = torch.empty(batch, dtype=momenta.dtype, device=momenta.device)
+    cur = torch.zeros((batch, m, m, d), dtype=momenta.dtype, device=momenta.device)
+    status = torch.zeros(batch, dtype=torch.int32, device=momenta.device)
+    s = (stream or torch.cuda.current_stream(momenta.device)).cuda_stream
+    with torch.cuda.device(momenta.device):
+        _check(bg_currents(field, n, d, batch, momenta.data_ptr(), polarisations.data_ptr(),
+                           out.data_ptr(), cur.data_ptr(), status.data_ptr(), s))
+    return out, cur, status
+
+
+def amplitudes_host(momenta: np.ndarray, polarisations: np.ndarray, workspace=None, out=None,
+                    status=None, chunk_points: int = 1 << 16):
+    """End-to-end call on HOST arrays (numpy, ideally backed by pinned memory): H2D copies,
+    kernel and D2H copies are pipelined inside the library."""
+    torch = _torch()
+    field = FIELD_FP31 if momenta.dtype == np.uint32 else FIELD_C128
+    batch, n, d = momenta.shape
+    if workspace is None:
+        nbytes = bg_host_workspace_bytes(field, n, d, max(1024, min(chunk_points, batch)))
+        workspace = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    if out is None:
+        out = np.empty(batch, dtype=momenta.dtype)
+    _check(bg_amplitudes_host(field, n, d, batch, momenta.ctypes.data, polarisations.ctypes.data,
+                              out.ctypes.data, None if status is None else status.ctypes.data,
+                              workspace.data_ptr(), workspace.numel()))
+    return out

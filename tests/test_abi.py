@@ -1,0 +1,92 @@
+"""CPU-side checks of the boundary: the C-ABI library builds, loads and exports every
+symbol include/bg.h declares; the formula-only entry points agree with SURVEY.md §8(d).
+No compute call is made here (no GPU)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+from paper_2502_07060_b200 import binding, build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build()
+    return binding.load()
+
+
+def test_every_declared_symbol_is_exported(lib):
+    hdr = open(os.path.join(ROOT, "include", "bg.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(bg_[a-z0-9_]+)\s*\(", hdr))
+    assert declared == set(binding.EXPORTS)
+    raw = ctypes.CDLL(build.LIB)
+    for name in declared:
+        assert getattr(raw, name) is not None
+
+
+def test_no_torch_types_in_the_header():
+    hdr = open(os.path.join(ROOT, "include", "bg.h")).read()
+    assert "torch" not in hdr.lower().replace("pytorch", "") and "at::" not in hdr
+
+
+def test_constants(lib):
+    assert binding.bg_modulus() == (1 << 31) - 1
+    assert "sm_100a" in binding.bg_version()
+    assert binding.bg_status_string(0) == "ok"
+    assert "argument" in binding.bg_status_string(-1)
+
+
+@pytest.mark.parametrize("n,d,field,mref,s3,s4,R,bytes_in", [
+    (4, 4, 0, 143, 4, 1, 2, 128),
+    (6, 4, 1, 940, 20, 15, 9, 768),
+    (8, 6, 0, 4839, 56, 70, 20, 384),
+    (10, 8, 0, 16510, 120, 210, 35, 640),
+    (12, 6, 0, 26553, 220, 495, 54, 576),
+    (12, 6, 1, 26553, 220, 495, 54, 2304),
+])
+def test_op_counts_match_the_survey_table(lib, n, d, field, mref, s3, s4, R, bytes_in):
+    """M_ref = 6d C(n,3) + 6d C(n,4) + dR + 3(R-1) + dR + d"""
+    oc = binding.bg_op_count(field, n, d)
+    assert oc["mul_ref"] == mref
+    assert (oc["splits3"], oc["splits4"], oc["propagators"]) == (s3, s4, R)
+    assert oc["currents"] == n * (n - 1) // 2
+    assert oc["bytes_in"] == bytes_in
+    assert oc["mul_factored"] < oc["mul_ref"] or n <= 5
+
+
+def test_kernel_info_and_bad_shapes(lib):
+    ki = binding.bg_kernel_info(0, 8, 6)
+    assert ki["specialised"] == 1 and ki["threads_per_block"] == 32
+    assert ki["smem_bytes_per_block"] <= 232448
+    assert binding.bg_kernel_info(0, 7, 6)["specialised"] == 0
+    big = binding.bg_kernel_info(1, 16, 16)          # largest record: fewer points per block
+    assert 1 <= big["threads_per_block"] < 32
+    for bad in [(0, 3, 4), (0, 17, 4), (0, 4, 3), (0, 4, 17), (2, 4, 4)]:
+        with pytest.raises(binding.BgError):
+            binding.bg_kernel_info(*bad)
+
+
+def test_host_workspace_formula(lib):
+    w = binding.bg_host_workspace_bytes(0, 8, 6, 1024)
+    assert w == 2 * (2 * 1024 * 48 * 4 + 1024 * 4 + 1024 * 4)
+    assert binding.bg_host_workspace_bytes(0, 3, 6, 1024) == 0
+
+
+def test_product_does_not_import_the_oracle():
+    """the product path must not route through the oracle (or any CPU fallback)"""
+    pkg = os.path.join(ROOT, "paper_2502_07060_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src, f
+                assert "bg_oracle" not in src and "bg_recursion.inc" not in src, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c", ".inc")):
+            src = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_2502_07060_b200" not in src and "from paper_2502_07060_b200" not in src, f
+            assert not re.search(r'#\s*include\s*[<"][^">]*(bg\.h|\.cuh)', src), f
