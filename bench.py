@@ -1,0 +1,425 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the Berends-Giele hot path on B200 (BASELINE.json's metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg2] [--impl reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 \
+        --master-port P bench.py --gpus N --steps K --warmup W
+
+A "step" is one pass of the whole hot path (SURVEY.md §8(a) rows a0-a6 = ONE kernel launch
+through the C ABI, `bg_amplitudes`) over one batch of seeded synthetic kinematics.  The
+headline workload is BASELINE.json configs[2] -- n=8 gluons, d=6, F_p (p=2^31-1), batch
+2^20 -- the configuration north_star's target is quoted on; `--config` selects another.
+With N GPUs every rank processes its own slice of N*batch points (points are independent:
+no collective on the data path, "scaling": "weak").
+
+Printed: ONE JSON line (rank 0) with the contract keys plus `roofline` (bound "alu": the
+modmul-bound line of SURVEY.md §8(d) / DESIGN.md §Roofline), `cpu_baseline` (the oracle as
+it stands, on this box's host cores, on a bounded sample), `e2e` (the same metric through
+`bg_amplitudes_host` with pinned HOST buffers, H2D/D2H copies inside the timed region),
+`clocks`, `gpu_launches`, and `per_config` (short device-resident timings of the other
+BASELINE.json configs, N=1 only; `--headline-only` skips them).
+`--impl reference` times the CPU oracle alone (this tier's reference arm).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_2502_07060_b200 import inputs  # noqa: E402
+
+METRIC = "amplitudes_per_second"
+UNIT = "amplitudes/s"
+# ALU-pipe bound of the canonical Mersenne-31 modular multiplication
+# (1 IMAD.WIDE on the FMA pipe + 3 ALU-pipe instructions; the ALU pipe issues 16 lanes per
+# clock per SM sub-partition = 64 per SM): 148 SMs x 64/3 per clock x max SM clock.
+SM_COUNT = 148
+ALU_LANES_PER_CLK_PER_SM = 64
+ALU_OPS_PER_MODMUL = 3
+DFMA_LANES_PER_CLK_PER_SM = 64      # checked against the DFMA probe
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+# ------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """samples SM clock and throttle reasons with NVML while the timed region runs"""
+
+    def __init__(self, index: int, period: float = 0.01):
+        self.samples, self.reasons, self.power = [], set(), []
+        self.period, self._stop, self._thr = period, threading.Event(), None
+        self.sm_max = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.sm_max = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception as e:  # noqa: BLE001
+            log(f"[bench] NVML unavailable ({e}); clocks not sampled")
+            self.nv = None
+
+    _NAMES = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+              0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+              0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                for bit, name in self._NAMES.items():
+                    if r & bit and name != "gpu_idle":
+                        self.reasons.add(name)
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+            except Exception:  # noqa: BLE001
+                pass
+            self._stop.wait(self.period)
+
+    def __enter__(self):
+        if self.nv:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        if self._thr:
+            self._thr.join()
+
+    def summary(self) -> dict:
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": [], "samples": 0}
+        return {"sm_mhz": statistics.median(self.samples), "sm_max_mhz": self.sm_max,
+                "reasons": sorted(self.reasons), "samples": len(self.samples),
+                "power_w_max": max(self.power) if self.power else None}
+
+
+# ------------------------------------------------------------------------------- helpers
+def op_counts(field: str, n: int, d: int) -> dict:
+    """M_ref of SURVEY.md §8(d) by formula (the C library exports the same via bg_op_count;
+    restated here so the reference arm needs no CUDA library)."""
+    from math import comb
+    m = n - 1
+    R = m * (m - 1) // 2 - 1
+    w = 4 if field == "fp31" else 16
+    return {"mul_ref": 6 * d * comb(n, 3) + 6 * d * comb(n, 4) + d * R + 3 * (R - 1) + d * R + d,
+            "bytes": 2 * n * d * w + w}
+
+
+def host_cores() -> int:
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+def time_oracle(cfg_name: str, sample_points: int, cores: int, repeats: int = 1, start: int = 0):
+    """the oracle as it stands, one thread per core over contiguous batch slices"""
+    import oracle
+    cfg = inputs.CONFIGS[cfg_name]
+    mom, pol, _ = inputs.make_config_threaded(cfg_name, batch=sample_points, start=start)
+    f = oracle.FP31 if cfg["field"] == "fp31" else oracle.C128
+    oracle.amplitudes(f, mom[:256], pol[:256], threads=1)        # load the library
+    ts = []
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        oracle.amplitudes(f, mom, pol, threads=cores)
+        ts.append(time.perf_counter() - t0)
+    return ts
+
+
+def pick_oracle_sample(cfg_name: str, cores: int, target_s: float) -> int:
+    """sample size giving about target_s seconds of oracle wall time on `cores` threads"""
+    probe = 256 * max(1, min(cores, 8))
+    t = time_oracle(cfg_name, probe, cores)[0]
+    pts = int(probe * target_s / max(t, 1e-6))
+    full = inputs.CONFIGS[cfg_name]["batch"]
+    return max(probe, min(full, 1 << max(8, pts.bit_length() - 1)))
+
+
+# ------------------------------------------------------------------------------- reference arm
+def run_reference(args) -> None:
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cores = host_cores()
+    name = args.config
+    cfg = inputs.CONFIGS[name]
+    sample = args.oracle_points or pick_oracle_sample(name, cores, 2.0)
+    total = args.steps + args.warmup
+    ts = time_oracle(name, sample, cores, repeats=total)
+    timed = ts[args.warmup:]
+    ms = 1e3 * sum(timed) / len(timed)
+    value = sample / (ms * 1e-3)
+    desc = f"{sample} points of {name} per step (the first points of the seeded workload), {cores} threads"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "u32" if cfg["field"] == "fp31" else "f64",
+        "data": "synthetic (seeded light-cone kinematics, DESIGN.md §Input recipe)",
+        "config": {"workload": workload_name(name), "sample_points_per_step": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def workload_name(name: str) -> str:
+    c = inputs.CONFIGS[name]
+    fld = "F_p(p=2^31-1)" if c["field"] == "fp31" else "complex128"
+    return f"{name}: n={c['n']} gluons, d={c['d']}, {fld}, batch {c['batch']} per GPU, seed 0"
+
+
+# ------------------------------------------------------------------------------- GPU arm
+def device_bench(binding, torch, name: str, batch: int, start: int, steps: int, warmup: int, dist):
+    """device-resident timing of `steps` launches; returns dict"""
+    cfg = inputs.CONFIGS[name]
+    t0 = time.perf_counter()
+    mom, pol, info = inputs.make_config_threaded(name, batch=batch, start=start)
+    gen_s = time.perf_counter() - t0
+    dm, dp = binding.to_device(mom), binding.to_device(pol)
+    out = torch.empty(batch, dtype=dm.dtype, device="cuda")
+    stream = torch.cuda.current_stream()
+    field = binding.field_of(dm)
+    n, d = cfg["n"], cfg["d"]
+
+    def launch():
+        rc = binding.bg_amplitudes(field, n, d, batch, dm.data_ptr(), dp.data_ptr(), out.data_ptr(),
+                                   stream.cuda_stream)
+        if rc != binding.BG_OK:
+            raise RuntimeError(f"bg_amplitudes failed: {binding.bg_status_string(rc)}")
+
+    for _ in range(warmup):
+        launch()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    evs[0].record(stream)
+    for k in range(steps):
+        launch()
+        evs[k + 1].record(stream)
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    total_ms = evs[0].elapsed_time(evs[-1])
+    per = [evs[k].elapsed_time(evs[k + 1]) for k in range(steps)]
+    return {"total_ms": total_ms, "per_launch_ms": per, "mom": mom, "pol": pol, "out": out,
+            "gen_s": gen_s, "redraws": info.get("redraws", 0), "dm": dm, "dp": dp}
+
+
+def e2e_bench(binding, torch, name: str, mom: np.ndarray, pol: np.ndarray, steps: int, warmup: int, dist):
+    """bg_amplitudes_host on pinned host buffers: H2D + kernel + D2H inside the timed region"""
+    cfg = inputs.CONFIGS[name]
+    batch = mom.shape[0]
+    field = binding.FIELD_FP31 if cfg["field"] == "fp31" else binding.FIELD_C128
+
+    def pinned(a):
+        t = torch.from_numpy(a.view(np.int32) if a.dtype == np.uint32 else a).pin_memory()
+        return t, t.numpy()
+
+    tm, hm = pinned(mom)
+    tp, hp = pinned(pol)
+    to = torch.empty(batch, dtype=tm.dtype).pin_memory()
+    ho = to.numpy()
+    chunk = min(batch, 1 << 17)
+    ws = torch.empty(binding.bg_host_workspace_bytes(field, cfg["n"], cfg["d"], chunk), dtype=torch.uint8,
+                     device="cuda")
+
+    def call():
+        rc = binding.bg_amplitudes_host(field, cfg["n"], cfg["d"], batch, hm.ctypes.data, hp.ctypes.data,
+                                        ho.ctypes.data, None, ws.data_ptr(), ws.numel())
+        if rc != binding.BG_OK:
+            raise RuntimeError(f"bg_amplitudes_host failed: {binding.bg_status_string(rc)}")
+
+    for _ in range(max(1, warmup)):
+        call()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        call()                      # returns after the results are in host memory
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    res = ho.view(np.uint32).copy() if cfg["field"] == "fp31" else ho.copy()
+    return {"s_per_step": dt / steps, "h2d": int(mom.nbytes + pol.nbytes), "d2h": int(ho.nbytes), "out": res}
+
+
+def roofline(field: str, n: int, d: int, batch: int, kernel_ms: float, sm_max_mhz: float, probes: dict | None,
+             traffic):
+    oc = op_counts(field, n, d)
+    clk = (sm_max_mhz or 1965.0) * 1e6
+    if field == "fp31":
+        peak = SM_COUNT * ALU_LANES_PER_CLK_PER_SM / ALU_OPS_PER_MODMUL * clk          # modmul/s
+        achieved = oc["mul_ref"] * batch / (kernel_ms * 1e-3)
+        unit, what = "Gmodmul/s", ("M_ref field multiplications of the literal Eq.(6) evaluation per amplitude "
+                                   "(SURVEY.md §8(d)) x points / kernel time; peak = ALU-pipe bound of the "
+                                   "canonical 4-instruction Mersenne-31 modmul at max SM clock (DESIGN.md §Roofline)")
+    else:
+        peak = SM_COUNT * DFMA_LANES_PER_CLK_PER_SM * clk                                # DFMA/s
+        achieved = 4 * oc["mul_ref"] * batch / (kernel_ms * 1e-3)
+        unit, what = "GDFMA/s", ("4 DFMA per complex multiply-add x M_ref x points / kernel time; peak = "
+                                 "FP64-pipe issue rate at max SM clock (DESIGN.md §Roofline)")
+    r = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": unit, "frac": achieved / peak,
+         "traffic": traffic, "peak_source": "derived (DESIGN.md §Roofline); MEASURED_PEAKS.json has no ALU peak",
+         "what": what, "mul_ref_per_amplitude": oc["mul_ref"], "kernel_ms": kernel_ms,
+         "hbm_frac": oc["bytes"] * batch / (kernel_ms * 1e-3) / 1e9 / hbm_peak()}
+    if probes:
+        key = "modmul" if field == "fp31" else "dfma"
+        r["probe_peak"] = probes[key]["ops_per_s"] / 1e9
+        r["frac_of_probe"] = achieved / probes[key]["ops_per_s"]
+    return r
+
+
+def hbm_peak() -> float:
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"])
+    except Exception:  # noqa: BLE001
+        return 6650.0
+
+
+def run_gpu(args) -> None:
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the Berends-Giele path has no CPU fallback")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist = dist_mod
+    from paper_2502_07060_b200 import binding, measure
+    binding.load()
+
+    name = args.config
+    cfg = inputs.CONFIGS[name]
+    batch = args.batch or cfg["batch"]
+    start = rank * batch                       # weak scaling: rank r owns points [r*batch, (r+1)*batch)
+    phys = torch.cuda.current_device()
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    nvml_index = int(vis.split(",")[phys]) if vis and all(v.strip().isdigit() for v in vis.split(",")) else phys
+
+    with ClockSampler(nvml_index) as clk:
+        res = device_bench(binding, torch, name, batch, start, args.steps, args.warmup, dist)
+    clocks = clk.summary()
+    total_ms = torch.tensor([res["total_ms"]], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
+    total_ms = float(total_ms.item())
+    ms_per_step = total_ms / args.steps
+    value = world * batch / (ms_per_step * 1e-3)
+    kernel_ms = sum(res["per_launch_ms"]) / len(res["per_launch_ms"])
+
+    # end to end through the host entry point
+    e2e_steps = max(3, min(args.steps, args.e2e_steps))
+    e2e = e2e_bench(binding, torch, name, res["mom"], res["pol"], e2e_steps, min(args.warmup, 3), dist)
+    e2e_t = torch.tensor([e2e["s_per_step"]], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(e2e_t, op=dist.ReduceOp.MAX)
+    e2e_value = world * batch / float(e2e_t.item())
+    same = np.array_equal(e2e["out"], binding.to_numpy(res["out"])) if cfg["field"] == "fp31" else \
+        bool(np.allclose(e2e["out"], binding.to_numpy(res["out"]), rtol=1e-12, atol=0))
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u32" if cfg["field"] == "fp31" else "f64",
+        "data": "synthetic (seeded light-cone kinematics, DESIGN.md §Input recipe)",
+        "config": {"workload": workload_name(name), "n": cfg["n"], "d": cfg["d"], "field": cfg["field"],
+                   "batch_per_gpu": batch, "global_batch": world * batch, "parallelism": f"dp{world} (batch sharding, "
+                   "no collective)", "l2": "inputs (%.0f MB per step) exceed the 126 MB L2; no flush needed" %
+                   ((res["mom"].nbytes + res["pol"].nbytes) / 1e6) if res["mom"].nbytes * 2 > 126e6 else
+                   "inputs fit L2: a 256 MB buffer is NOT flushed between steps (arithmetic-bound kernel)",
+                   "redraws": res["redraws"]},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
+                "steps": e2e_steps, "matches_device_path": same,
+                "api": "bg_amplitudes_host (pinned host buffers, chunked H2D/kernel/D2H pipeline)"},
+        "gpu_launches": args.steps,
+        "clocks": clocks,
+        "kernel": binding.bg_kernel_info(binding.FIELD_FP31 if cfg["field"] == "fp31" else binding.FIELD_C128,
+                                         cfg["n"], cfg["d"]),
+    }
+
+    if rank == 0:
+        probes = None
+        if not args.no_probes:
+            probes = measure.measure_peaks(kinds=["imad_wide", "alu", "mix", "modmul", "dfma", "lds64"])
+            line["pipe_probes_Gops"] = {k: round(v["ops_per_s"] / 1e9, 1) for k, v in probes.items()
+                                        if isinstance(v, dict)}
+        line["roofline"] = roofline(cfg["field"], cfg["n"], cfg["d"], batch, kernel_ms, clocks.get("sm_max_mhz"),
+                                    probes, args.traffic)
+        if world == 1 and not args.headline_only:
+            per = []
+            for other in inputs.CONFIGS:
+                if other == name:
+                    continue
+                oc = inputs.CONFIGS[other]
+                r = device_bench(binding, torch, other, oc["batch"], 0, args.config_steps, 3, None)
+                kms = statistics.median(r["per_launch_ms"])
+                rl = roofline(oc["field"], oc["n"], oc["d"], oc["batch"], kms, clocks.get("sm_max_mhz"), probes, None)
+                per.append({"workload": workload_name(other), "value": oc["batch"] / (kms * 1e-3), "unit": UNIT,
+                            "kernel_ms_median": kms, "launches": args.config_steps,
+                            "roofline_frac": rl["frac"], "roofline_unit": rl["unit"], "hbm_frac": rl["hbm_frac"]})
+                del r
+            line["per_config"] = per
+        if world == 1 and not args.no_cpu_baseline:
+            cores = host_cores()
+            sample = args.oracle_points or pick_oracle_sample(name, cores, 10.0)
+            t = time_oracle(name, sample, cores)[0]
+            line["cpu_baseline"] = {"value": sample / t, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "sample": f"the first {sample} points of {name} (same seeded workload), "
+                                              f"{t:.1f} s on {cores} threads"}
+        print(json.dumps(line))
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="cfg2", choices=list(inputs.CONFIGS))
+    ap.add_argument("--batch", type=int, default=0, help="points per GPU (default: the config's batch)")
+    ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--config-steps", type=int, default=20, help="launches per secondary config")
+    ap.add_argument("--oracle-points", type=int, default=0)
+    ap.add_argument("--headline-only", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-probes", action="store_true")
+    ap.add_argument("--traffic", type=float, default=None,
+                    help="dram bytes per launch of the recursion kernel from the committed ncu capture "
+                         "(profiles/); reported as roofline.traffic")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        log("[bench] note: fewer than 3 warm-up steps requested")
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

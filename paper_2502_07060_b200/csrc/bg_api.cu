@@ -6,6 +6,8 @@
 
 #include "../../include/bg.h"
 #include "bg_recursion.cuh"
+#include "bg_sweep.cuh"
+#include <stdlib.h>
 
 namespace {
 
@@ -95,6 +97,50 @@ const void* pick(int n, int d, int* s)
     return nullptr;
 }
 
+// ---- the compile-time (n, d) fast path: bg_sweep_kernel<F, N, D, W> ---------------------------
+struct SweepEntry {
+    int field, n, d, w;
+    const void* func;
+    size_t smem;
+};
+
+template <class F, int N, int D, int W>
+SweepEntry sweep_entry(int field)
+{
+    return SweepEntry{field, N, D, W, reinterpret_cast<const void*>(&bg::bg_sweep_kernel<F, N, D, W>),
+                      bg::SweepCfg<F, N, D, W>::SMEM_BYTES};
+}
+
+// first entry of a shape = the default warps-per-tile; the others can be selected with the
+// tuning knob BG_SWEEP_W (environment, read per call; used by the benchmarks' sweeps)
+const SweepEntry* sweep_table(int* count)
+{
+    static const SweepEntry table[] = {
+        sweep_entry<Fp31, 8, 6, 4>(BG_FIELD_FP31),
+        sweep_entry<Fp31, 8, 6, 1>(BG_FIELD_FP31),
+        sweep_entry<Fp31, 8, 6, 2>(BG_FIELD_FP31),
+    };
+    *count = (int)(sizeof(table) / sizeof(table[0]));
+    return table;
+}
+
+const SweepEntry* find_sweep(int field, int n, int d)
+{
+    int count = 0;
+    const SweepEntry* t = sweep_table(&count);
+    const char* env = getenv("BG_SWEEP_W");
+    const int want = env ? atoi(env) : 0;
+    if (env && want == 0) return nullptr;            // BG_SWEEP_W=0: force the runtime-n kernel
+    const SweepEntry* first = nullptr;
+    for (int i = 0; i < count; ++i) {
+        if (t[i].field != field || t[i].n != n || t[i].d != d) continue;
+        if (t[i].smem > (size_t)kMaxSmemPerBlock) continue;
+        if (!first) first = &t[i];
+        if (t[i].w == want) return &t[i];
+    }
+    return first;
+}
+
 int vec_width(int field, int d)
 {
     if (field == BG_FIELD_C128) return 1;
@@ -157,6 +203,31 @@ int launch_typed(const LaunchPlan& plan, int n, int64_t batch, const void* mom, 
     return BG_OK;
 }
 
+template <class E>
+int launch_sweep(const SweepEntry& e, int64_t batch, const void* mom, const void* pol, void* out, void* cur,
+                 uint32_t* status, cudaStream_t stream)
+{
+    bg::SweepParams<E> prm;
+    prm.mom = static_cast<const E*>(mom);
+    prm.pol = static_cast<const E*>(pol);
+    prm.out = static_cast<E*>(out);
+    prm.currents = static_cast<E*>(cur);
+    prm.status = status;
+    prm.batch = batch;
+    if (cudaFuncSetAttribute(e.func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)e.smem) != cudaSuccess) {
+        cudaGetLastError();
+        return BG_ERR_CUDA;
+    }
+    const int64_t blocks = (batch + 31) / 32;
+    if (blocks > 0x7fffffffLL) return BG_ERR_ARG;
+    void* args[] = {&prm};
+    if (cudaLaunchKernel(e.func, dim3((unsigned)blocks), dim3(32 * e.w), args, e.smem, stream) != cudaSuccess) {
+        cudaGetLastError();
+        return BG_ERR_CUDA;
+    }
+    return BG_OK;
+}
+
 int run(int field, int n, int d, int64_t batch, const void* mom, const void* pol, void* out, void* cur,
         uint32_t* status, cudaStream_t stream)
 {
@@ -170,6 +241,10 @@ int run(int field, int n, int d, int64_t batch, const void* mom, const void* pol
         (reinterpret_cast<uintptr_t>(status) & 3u))
         return BG_ERR_ARG;
     if (out == mom || out == pol) return BG_ERR_ARG;
+    if (const SweepEntry* e = find_sweep(field, n, d)) {
+        if (field == BG_FIELD_FP31) return launch_sweep<uint32_t>(*e, batch, mom, pol, out, cur, status, stream);
+        return launch_sweep<double2>(*e, batch, mom, pol, out, cur, status, stream);
+    }
     if (field == BG_FIELD_FP31)
         return launch_typed<uint32_t>(plan, n, batch, mom, pol, out, cur, status, stream);
     return launch_typed<double2>(plan, n, batch, mom, pol, out, cur, status, stream);

@@ -24,6 +24,11 @@ namespace bg {
 
 constexpr uint32_t kP = 0x7fffffffu;
 
+// 2^32 mod p, read from constant memory so that it stays opaque to ptxas: with a literal 2
+// the fold `hi * 2 + lo` is strength-reduced into five shift/add instructions instead of the
+// single IMAD.WIDE.U32 it is meant to be.
+__constant__ uint32_t c_two32 = 2u;
+
 struct Fp31 {
     typedef uint32_t E;   // element
     typedef uint64_t A;   // lazy accumulator
@@ -39,12 +44,21 @@ struct Fp31 {
     __device__ __forceinline__ static E ezero() { return 0u; }
     __device__ __forceinline__ static E one() { return 1u; }
     __device__ __forceinline__ static bool is_zero(E a) { return a == 0u; }
-    __device__ __forceinline__ static A mad(E a, E b, A c) { return (uint64_t)a * b + c; }
+    // a*b + c as ONE IMAD.WIDE.U32 (inline PTX: left to itself the compiler re-associates the
+    // sums and strength-reduces the fold's multiplication by 2 into five shift/add instructions)
+    __device__ __forceinline__ static A mad(E a, E b, A c)
+    {
+        A d;
+        asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(d) : "r"(a), "r"(b), "l"(c));
+        return d;
+    }
     __device__ __forceinline__ static A widen(E a) { return (uint64_t)a; }
+    __device__ __forceinline__ static A accumulate(A c, E a) { return c + (uint64_t)a; }
+    __device__ __forceinline__ static E half() { return 0x40000000u; }          // 2^-1 = 2^30
     // x = hi 2^32 + lo = 2 hi + lo (mod p): one IMAD.WIDE.U32, result < 3*2^32
     __device__ __forceinline__ static A fold(A x)
     {
-        return (uint64_t)(uint32_t)(x >> 32) * 2u + (uint32_t)x;
+        return mad((uint32_t)(x >> 32), c_two32, (uint64_t)(uint32_t)x);
     }
     // canonical residue of y < 2^62 + 2^33 (so that (y>>31) + (y&p) < 2^32)
     __device__ __forceinline__ static E reduce62(A y)
@@ -128,6 +142,8 @@ struct C128 {
         return make_double2(re, im);
     }
     __device__ __forceinline__ static A widen(E a) { return a; }
+    __device__ __forceinline__ static A accumulate(A c, E a) { return make_double2(c.x + a.x, c.y + a.y); }
+    __device__ __forceinline__ static E half() { return make_double2(0.5, 0.0); }
     __device__ __forceinline__ static A fold(A x) { return x; }
     __device__ __forceinline__ static E reduce(A x) { return x; }
     __device__ __forceinline__ static E reduce_half(A x) { return make_double2(0.5 * x.x, 0.5 * x.y); }

@@ -62,6 +62,20 @@ __host__ __device__ constexpr RecordLayout make_layout(int n, int d, int vec)
 template <class F, int D> struct VecWidth { static constexpr int value = 1; };
 template <int D> struct VecWidth<Fp31, D> { static constexpr int value = (D % 4 == 0) ? 4 : (D % 2 == 0) ? 2 : 1; };
 
+// the memory type of one vector unit of U elements, and the input reduction applied to it
+template <class F, int U> struct VecType { typedef typename F::E type; };
+template <> struct VecType<Fp31, 2> { typedef uint2 type; };
+template <> struct VecType<Fp31, 4> { typedef uint4 type; };
+template <class F> __device__ __forceinline__ typename F::E load_unit(typename F::E v) { return F::load_input(v); }
+template <class F> __device__ __forceinline__ uint2 load_unit(uint2 v)
+{
+    return make_uint2(F::load_input(v.x), F::load_input(v.y));
+}
+template <class F> __device__ __forceinline__ uint4 load_unit(uint4 v)
+{
+    return make_uint4(F::load_input(v.x), F::load_input(v.y), F::load_input(v.z), F::load_input(v.w));
+}
+
 template <class F, int D>
 __device__ __forceinline__ void ld_vec(const typename F::E* p, typename F::E (&v)[D])
 {

@@ -316,3 +316,24 @@ def make_config(name: str, batch: int | None = None, seed: int = 0, start: int =
     c = CONFIGS[name]
     return make_inputs(c["field"], c["n"], c["d"], c["batch"] if batch is None else batch,
                        seed, start, c["helicities"])
+
+
+def make_config_threaded(name: str, batch: int | None = None, seed: int = 0, start: int = 0,
+                         threads: int | None = None, chunk: int = 1 << 13):
+    """make_config() with the batch cut into chunks generated on a thread pool (numpy releases
+    the GIL on the large array operations).  Every draw is a pure function of (seed, global
+    point index), so the result is identical to the single-threaded call."""
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+    c = CONFIGS[name]
+    batch = c["batch"] if batch is None else batch
+    threads = threads or min(32, os.cpu_count() or 1)
+    if batch <= chunk or threads <= 1:
+        return make_config(name, batch, seed, start)
+    offs = list(range(0, batch, chunk))
+    with ThreadPoolExecutor(threads) as ex:
+        parts = list(ex.map(lambda o: make_config(name, min(chunk, batch - o), seed, start + o), offs))
+    mom = np.concatenate([p[0] for p in parts])
+    pol = np.concatenate([p[1] for p in parts])
+    info = {"redraws": sum(p[2]["redraws"] for p in parts)}
+    return mom, pol, info
