@@ -308,13 +308,13 @@ def run_gpu(args) -> None:
         import torch.distributed as dist_mod
         dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local))
         dist = dist_mod
-    from paper_2502_07060_b200 import binding, measure
+    from paper_2502_07060_b200 import binding, measure, sharding
     binding.load()
 
     name = args.config
     cfg = inputs.CONFIGS[name]
     batch = args.batch or cfg["batch"]
-    start = rank * batch                       # weak scaling: rank r owns points [r*batch, (r+1)*batch)
+    start, _ = sharding.weak_slice(rank, world, batch)   # rank r owns points [r*batch, (r+1)*batch)
     phys = torch.cuda.current_device()
     vis = os.environ.get("CUDA_VISIBLE_DEVICES")
     nvml_index = int(vis.split(",")[phys]) if vis and all(v.strip().isdigit() for v in vis.split(",")) else phys
