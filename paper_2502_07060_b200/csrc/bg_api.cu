@@ -6,7 +6,7 @@
 
 #include "../../include/bg.h"
 #include "bg_recursion.cuh"
-#include "bg_sweep.cuh"
+#include "bg_tile.cuh"
 #include <stdlib.h>
 
 namespace {
@@ -107,8 +107,8 @@ struct SweepEntry {
 template <class F, int N, int D, int W>
 SweepEntry sweep_entry(int field)
 {
-    return SweepEntry{field, N, D, W, reinterpret_cast<const void*>(&bg::bg_sweep_kernel<F, N, D, W>),
-                      bg::SweepCfg<F, N, D, W>::SMEM_BYTES};
+    return SweepEntry{field, N, D, W, reinterpret_cast<const void*>(&bg::bg_tile_kernel<F, N, D, W>),
+                      bg::TileCfg<F, N, D, W>::SMEM_BYTES};
 }
 
 // first entry of a shape = the default warps-per-tile; the others can be selected with the
@@ -119,6 +119,16 @@ const SweepEntry* sweep_table(int* count)
         sweep_entry<Fp31, 8, 6, 4>(BG_FIELD_FP31),
         sweep_entry<Fp31, 8, 6, 1>(BG_FIELD_FP31),
         sweep_entry<Fp31, 8, 6, 2>(BG_FIELD_FP31),
+        sweep_entry<Fp31, 8, 6, 8>(BG_FIELD_FP31),
+        sweep_entry<Fp31, 4, 4, 1>(BG_FIELD_FP31),
+        sweep_entry<Fp31, 10, 8, 8>(BG_FIELD_FP31),
+        sweep_entry<Fp31, 10, 8, 4>(BG_FIELD_FP31),
+        sweep_entry<Fp31, 12, 6, 8>(BG_FIELD_FP31),
+        sweep_entry<Fp31, 12, 6, 16>(BG_FIELD_FP31),
+        sweep_entry<Fp31, 12, 6, 4>(BG_FIELD_FP31),
+        sweep_entry<C128, 6, 4, 4>(BG_FIELD_C128),
+        sweep_entry<C128, 6, 4, 2>(BG_FIELD_C128),
+        sweep_entry<C128, 6, 4, 8>(BG_FIELD_C128),
     };
     *count = (int)(sizeof(table) / sizeof(table[0]));
     return table;
@@ -207,7 +217,7 @@ template <class E>
 int launch_sweep(const SweepEntry& e, int64_t batch, const void* mom, const void* pol, void* out, void* cur,
                  uint32_t* status, cudaStream_t stream)
 {
-    bg::SweepParams<E> prm;
+    bg::TileParams<E> prm;
     prm.mom = static_cast<const E*>(mom);
     prm.pol = static_cast<const E*>(pol);
     prm.out = static_cast<E*>(out);

@@ -44,14 +44,11 @@ struct Fp31 {
     __device__ __forceinline__ static E ezero() { return 0u; }
     __device__ __forceinline__ static E one() { return 1u; }
     __device__ __forceinline__ static bool is_zero(E a) { return a == 0u; }
-    // a*b + c as ONE IMAD.WIDE.U32 (inline PTX: left to itself the compiler re-associates the
-    // sums and strength-reduces the fold's multiplication by 2 into five shift/add instructions)
-    __device__ __forceinline__ static A mad(E a, E b, A c)
-    {
-        A d;
-        asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(d) : "r"(a), "r"(b), "l"(c));
-        return d;
-    }
+    // a*b + c: written as mul.wide + 64-bit add, which ptxas fuses into ONE IMAD.WIDE.U32 with a
+    // 64-bit addend and keeps as a serial chain.  (An inline-PTX mad.wide.u32 is instead split
+    // into IMAD.WIDE(..,RZ) + IADD3 + IADD3.X and re-associated: 1.9x the instructions,
+    // profiles/r01a_cfg2_sweep_w4_opmix.txt.)
+    __device__ __forceinline__ static A mad(E a, E b, A c) { return (uint64_t)a * b + c; }
     __device__ __forceinline__ static A widen(E a) { return (uint64_t)a; }
     __device__ __forceinline__ static A accumulate(A c, E a) { return c + (uint64_t)a; }
     __device__ __forceinline__ static E half() { return 0x40000000u; }          // 2^-1 = 2^30
