@@ -117,18 +117,12 @@ const SweepEntry* sweep_table(int* count)
 {
     static const SweepEntry table[] = {
         sweep_entry<Fp31, 8, 6, 4>(BG_FIELD_FP31),
-        sweep_entry<Fp31, 8, 6, 1>(BG_FIELD_FP31),
-        sweep_entry<Fp31, 8, 6, 2>(BG_FIELD_FP31),
         sweep_entry<Fp31, 8, 6, 8>(BG_FIELD_FP31),
         sweep_entry<Fp31, 4, 4, 1>(BG_FIELD_FP31),
         sweep_entry<Fp31, 10, 8, 8>(BG_FIELD_FP31),
-        sweep_entry<Fp31, 10, 8, 4>(BG_FIELD_FP31),
         sweep_entry<Fp31, 12, 6, 8>(BG_FIELD_FP31),
-        sweep_entry<Fp31, 12, 6, 16>(BG_FIELD_FP31),
-        sweep_entry<Fp31, 12, 6, 4>(BG_FIELD_FP31),
         sweep_entry<C128, 6, 4, 4>(BG_FIELD_C128),
         sweep_entry<C128, 6, 4, 2>(BG_FIELD_C128),
-        sweep_entry<C128, 6, 4, 8>(BG_FIELD_C128),
     };
     *count = (int)(sizeof(table) / sizeof(table[0]));
     return table;

@@ -52,10 +52,21 @@ struct Fp31 {
     __device__ __forceinline__ static A widen(E a) { return (uint64_t)a; }
     __device__ __forceinline__ static A accumulate(A c, E a) { return c + (uint64_t)a; }
     __device__ __forceinline__ static E half() { return 0x40000000u; }          // 2^-1 = 2^30
-    // x = hi 2^32 + lo = 2 hi + lo (mod p): one IMAD.WIDE.U32, result < 3*2^32
+    // x = hi 2^32 + lo = 2 hi + lo (mod p), result < 3*2^32.  Written in place -- add 2 hi to
+    // the whole accumulator (one IMAD.WIDE.U32), then take hi off the upper word (one IADD) --
+    // so that no register pair has to be rebuilt around the low word.
     __device__ __forceinline__ static A fold(A x)
     {
-        return mad((uint32_t)(x >> 32), c_two32, (uint64_t)(uint32_t)x);
+        // the word split / join is opaque inline PTX (register renaming only) so that the
+        // compiler cannot rewrite this back into "rebuild (lo, 0), then multiply-add"
+        uint32_t lo, hi, tl, th;
+        asm("mov.b64 {%0, %1}, %2;" : "=r"(lo), "=r"(hi) : "l"(x));
+        const A t = mad(hi, c_two32, x);
+        asm("mov.b64 {%0, %1}, %2;" : "=r"(tl), "=r"(th) : "l"(t));
+        th -= hi;
+        A r;
+        asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(tl), "r"(th));
+        return r;
     }
     // canonical residue of y < 2^62 + 2^33 (so that (y>>31) + (y&p) < 2^32)
     __device__ __forceinline__ static E reduce62(A y)

@@ -37,6 +37,13 @@ struct TileItem {
     uint32_t x, y;
 };
 
+// The form the kernel reads: byte offsets into the per-point vector record, ready for use as
+// [base + offset] operands (independent of W), and the chunk-dependent flags on the side.
+struct alignas(16) TileOff {
+    uint32_t a, b, c;      // byte offsets of the three vector rows (c: PS2_k row for a 3-split)
+    uint32_t uv;           // 3-split: byte offset of U_A | byte offset of V_B << 16 in the lane's scalar column
+};
+
 template <int N, int W>
 struct TileTables {
     static constexpr int M = N - 1;
@@ -45,6 +52,20 @@ struct TileTables {
     TileItem items[NITEMS];
     uint16_t beg[M + 1][W + 1];          // warp w of level L owns items [beg[L][w], beg[L][w+1])
     TileItem jobs[M + 1][MAXJOBS];       // x: slot mask;  y: as in TileItem (slot unused)
+    uint8_t njobs[M + 1];
+};
+
+// what lands in constant memory
+template <int N, int W>
+struct TileProgram {
+    static constexpr int M = N - 1;
+    static constexpr int NITEMS = TileTables<N, W>::NITEMS;
+    TileOff off[NITEMS];
+    uint32_t seg[NITEMS];                // lo | hi << 8 | own_row << 16 | slot << 24
+    uint16_t flags[NITEMS];
+    uint16_t beg[M + 1][W + 1];
+    uint32_t job_mask[M + 1][W];
+    uint32_t job_seg[M + 1][W];
     uint8_t njobs[M + 1];
 };
 
@@ -151,6 +172,34 @@ constexpr TileTables<N, W> make_tile_tables()
         base += cnt;
     }
     return t;
+}
+
+// rowbytes = D * sizeof(E); ps0 = first PS2 row; sc_u, sc_v = first scalar index of the U / V tables;
+// scalbytes = 32 * sizeof(E), the distance between consecutive scalars of one lane
+template <int N, int W>
+constexpr TileProgram<N, W> make_tile_program(int rowbytes, int ps0, int sc_u, int sc_v, int scalbytes)
+{
+    const TileTables<N, W> t = make_tile_tables<N, W>();
+    TileProgram<N, W> p{};
+    for (int q = 0; q < TileTables<N, W>::NITEMS; ++q) {
+        const uint32_t x = t.items[q].x;
+        const uint32_t a = x & 255u, b = x >> 8 & 255u, c = x >> 16 & 255u, fl = x >> 24;
+        p.off[q].a = a * rowbytes;
+        p.off[q].b = b * rowbytes;
+        p.off[q].c = ((fl & IT_KIND4) ? c : ps0 + c) * rowbytes;
+        p.off[q].uv = (fl & IT_KIND4) ? 0u : (uint32_t)((sc_u + a) * scalbytes) | (uint32_t)((sc_v + b) * scalbytes) << 16;
+        p.seg[q] = t.items[q].y;
+        p.flags[q] = (uint16_t)fl;
+    }
+    for (int L = 0; L <= N - 1; ++L) {
+        for (int w = 0; w <= W; ++w) p.beg[L][w] = t.beg[L][w];
+        p.njobs[L] = t.njobs[L];
+        for (int j = 0; j < W; ++j) {
+            p.job_mask[L][j] = t.jobs[L][j].x;
+            p.job_seg[L][j] = t.jobs[L][j].y;
+        }
+    }
+    return p;
 }
 
 }  // namespace bg

@@ -53,9 +53,11 @@ struct TileCfg {
     static constexpr size_t SMEM_BYTES = (size_t)32 * (VSTRIDE + NSCAL) * sizeof(E) + 32 * sizeof(uint32_t);
 };
 
-// the tables of one (N, W) instance, in constant memory
-template <int N, int W>
-__constant__ TileTables<N, W> c_tile_tables = make_tile_tables<N, W>();
+// the work lists of one (field, N, D, W) instance, in constant memory
+template <class F, int N, int D, int W>
+__constant__ TileProgram<N, W> c_tile_program = make_tile_program<N, W>(
+    D * (int)sizeof(typename F::E), TileCfg<F, N, D, W>::PS0, TileCfg<F, N, D, W>::SC_U, TileCfg<F, N, D, W>::SC_V,
+    32 * (int)sizeof(typename F::E));
 
 template <class E>
 struct TileParams {
@@ -129,9 +131,11 @@ __global__ void __launch_bounds__(32 * W) bg_tile_kernel(const TileParams<typena
     E* vec = reinterpret_cast<E*>(smem_raw);                  // [32][VSTRIDE]
     E* scal = vec + 32 * C::VSTRIDE;                          // [NSCAL][32]
     uint32_t* stat = reinterpret_cast<uint32_t*>(scal + 32 * C::NSCAL);
-    const TileTables<N, W>& tb = c_tile_tables<N, W>;
+    const TileProgram<N, W>& tb = c_tile_program<F, N, D, W>;
 
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // the warp index, broadcast from lane 0 so that everything derived from it (chunk bounds,
+    // item words, branch conditions) is compiled as warp-uniform
+    const int lane = threadIdx.x & 31, warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
     const long long tile0 = (long long)blockIdx.x * 32;
     const int valid = (int)min(32LL, prm.batch - tile0);
     const long long pt = tile0 + lane;
@@ -255,12 +259,15 @@ __global__ void __launch_bounds__(32 * W) bg_tile_kernel(const TileParams<typena
         for (int mu = 0; mu < D; ++mu) { acc[mu] = F::zero(); a[mu] = F::ezero(); x2[mu] = F::ezero(); }
 #pragma unroll 1
         for (int it = ibeg; it < iend; ++it) {
-            const uint32_t wx = tb.items[it].x, wy = tb.items[it].y;
-            const int lo = wy & 255, hi = wy >> 8 & 255;
-            if (wx & IT_SEG_START << 24) {
+            const uint32_t fl = tb.flags[it];
+            const TileOff o = tb.off[it];
+            const char* recb = reinterpret_cast<const char*>(rec);
+            const char* scb = reinterpret_cast<const char*>(sc);
+            if (fl & IT_SEG_START) {
+                const uint32_t sg = tb.seg[it];
                 E l[D], h[D];
-                ld_vec<F, D>(rec + (C::PS0 + lo) * D, l);
-                ld_vec<F, D>(rec + (C::PS0 + hi) * D, h);
+                ld_vec<F, D>(rec + (C::PS0 + (sg & 255)) * D, l);
+                ld_vec<F, D>(rec + (C::PS0 + (sg >> 8 & 255)) * D, h);
                 x2[0] = F::sub(h[0], l[0]);                          // 2 * covariant P_{i,j}
 #pragma unroll
                 for (int mu = 1; mu < D; ++mu) x2[mu] = F::sub(l[mu], h[mu]);
@@ -269,18 +276,17 @@ __global__ void __launch_bounds__(32 * W) bg_tile_kernel(const TileParams<typena
                 hsum = F::ezero();
                 room = F::kCap;
             }
-            if (wx & IT_LOAD_A << 24) {
-                ld_vec<F, D>(rec + (wx & 255) * D, a);
+            if (fl & IT_LOAD_A) {
+                ld_vec<F, D>(reinterpret_cast<const E*>(recb + o.a), a);
                 na0 = F::neg(a[0]);
             }
-            const E* brow = rec + (wx >> 8 & 255) * D;
-            if (!(wx & IT_KIND4 << 24)) {
+            if (!(fl & IT_KIND4)) {
                 // ---- 3-gluon split (i..k | k+1..j) -------------------------------------------------
                 E b[D], s[D];
-                ld_vec<F, D>(brow, b);
-                ld_vec<F, D>(rec + (C::PS0 + (wx >> 16 & 255)) * D, s);
-                const E ua = sc[(C::SC_U + (wx & 255)) * 32];
-                const E vb = sc[(C::SC_V + (wx >> 8 & 255)) * 32];
+                ld_vec<F, D>(reinterpret_cast<const E*>(recb + o.b), b);
+                ld_vec<F, D>(reinterpret_cast<const E*>(recb + o.c), s);
+                const E ua = *reinterpret_cast<const E*>(scb + (o.uv & 0xffffu));
+                const E vb = *reinterpret_cast<const E*>(scb + (o.uv >> 16));
                 const E h = F::neg(F::reduce(dot_neg<F, D>(na0, a, b)));          // A.B
                 const E xa = F::reduce(dot_plain<F, D>(x2, a));                   // 2 X.A
                 const E xb = F::reduce(dot_plain<F, D>(x2, b));                   // 2 X.B
@@ -302,8 +308,8 @@ __global__ void __launch_bounds__(32 * W) bg_tile_kernel(const TileParams<typena
             } else {
                 // ---- 4-gluon split (i..k | k+1..l | l+1..j): 2 (A.C) J(k+1..l) ------------------------
                 E bm[D], c[D];
-                ld_vec<F, D>(brow, bm);
-                ld_vec<F, D>(rec + (wx >> 16 & 255) * D, c);
+                ld_vec<F, D>(reinterpret_cast<const E*>(recb + o.b), bm);
+                ld_vec<F, D>(reinterpret_cast<const E*>(recb + o.c), c);
                 const E cc = F::neg(F::dbl(F::reduce(dot_neg<F, D>(na0, a, c))));   // 2 A.C
                 if (room < 1) {
 #pragma unroll
@@ -314,12 +320,13 @@ __global__ void __launch_bounds__(32 * W) bg_tile_kernel(const TileParams<typena
 #pragma unroll
                 for (int mu = 0; mu < D; ++mu) acc[mu] = F::mad(cc, bm[mu], acc[mu]);
             }
-            if (wx & IT_SEG_END << 24) {
-                if (wx & IT_COMPLETE << 24) {
-                    tile_finish<F, N, D, W>(rec, sc, acc, hsum, wy >> 16 & 255, lo, hi, (wx & IT_TOP << 24) != 0,
+            if (fl & IT_SEG_END) {
+                const uint32_t sg = tb.seg[it];
+                if (fl & IT_COMPLETE) {
+                    tile_finish<F, N, D, W>(rec, sc, acc, hsum, sg >> 16 & 255, sg & 255, sg >> 8 & 255, L == M,
                                             prm, pt, live);
                 } else {
-                    E* scr = sc + (C::SC_SCR + (wy >> 24) * (D + 1)) * 32;
+                    E* scr = sc + (C::SC_SCR + (sg >> 24) * (D + 1)) * 32;
 #pragma unroll
                     for (int mu = 0; mu < D; ++mu) scr[mu * 32] = F::reduce(acc[mu]);
                     scr[D * 32] = hsum;
@@ -332,8 +339,8 @@ __global__ void __launch_bounds__(32 * W) bg_tile_kernel(const TileParams<typena
             __syncthreads();
 #pragma unroll 1
             for (int j = warp; j < nj; j += W) {
-                uint32_t mask = tb.jobs[L][j].x;
-                const uint32_t wy = tb.jobs[L][j].y;
+                uint32_t mask = tb.job_mask[L][j];
+                const uint32_t wy = tb.job_seg[L][j];
 #pragma unroll
                 for (int mu = 0; mu < D; ++mu) acc[mu] = F::zero();
                 hsum = F::ezero();
