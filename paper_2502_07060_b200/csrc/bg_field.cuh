@@ -33,6 +33,8 @@ struct Fp31 {
     typedef uint32_t E;   // element
     typedef uint64_t A;   // lazy accumulator
     static constexpr int kCap = 4;            // products an accumulator takes between folds
+    static constexpr int kCap0 = 4;           // products an accumulator takes starting from zero
+    static constexpr int kCapR = 2;           // products an accumulator takes after relief()
     static constexpr bool kExact = true;
 
     __device__ __forceinline__ static E load_input(uint32_t raw)
@@ -66,6 +68,22 @@ struct Fp31 {
         th -= hi;
         A r;
         asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(tl), "r"(th));
+        return r;
+    }
+    // Headroom without touching the multiplier pipe: subtract p 2^32 (= 0 mod p) when the upper
+    // word allows it, hi <- min(hi, hi - p) (unsigned): ONE ALU instruction (VIADDMNMX.U32).
+    // A product of an operand <= p with one <= p-1 raises the upper word by at most 2^30 - 1
+    // (carry included), so from zero an accumulator takes kCap0 = 4 products (hi <= 2^32 - 4),
+    // relief() brings hi <= 2^31 - 2, and every relief() buys kCapR = 2 more products.
+    // (IMAD.WIDE.U32 issues at a quarter of the ALU rate on sm_100 -- profiles/r01b -- so the
+    // fold above, one more IMAD.WIDE, is kept for the final reduce only.)
+    __device__ __forceinline__ static A relief(A x)
+    {
+        uint32_t lo, hi;
+        asm("mov.b64 {%0, %1}, %2;" : "=r"(lo), "=r"(hi) : "l"(x));
+        hi = min(hi, hi - kP);
+        A r;
+        asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(lo), "r"(hi));
         return r;
     }
     // canonical residue of y < 2^62 + 2^33 (so that (y>>31) + (y&p) < 2^32)
@@ -134,6 +152,8 @@ struct C128 {
     typedef double2 E;
     typedef double2 A;
     static constexpr int kCap = 1 << 30;      // never needs folding
+    static constexpr int kCap0 = 1 << 30;
+    static constexpr int kCapR = 1 << 30;
     static constexpr bool kExact = false;
 
     __device__ __forceinline__ static E load_input(double2 raw) { return raw; }
@@ -153,6 +173,7 @@ struct C128 {
     __device__ __forceinline__ static A accumulate(A c, E a) { return make_double2(c.x + a.x, c.y + a.y); }
     __device__ __forceinline__ static E half() { return make_double2(0.5, 0.0); }
     __device__ __forceinline__ static A fold(A x) { return x; }
+    __device__ __forceinline__ static A relief(A x) { return x; }
     __device__ __forceinline__ static E reduce(A x) { return x; }
     __device__ __forceinline__ static E reduce_half(A x) { return make_double2(0.5 * x.x, 0.5 * x.y); }
     __device__ __forceinline__ static E reduce_double(A x) { return make_double2(2.0 * x.x, 2.0 * x.y); }

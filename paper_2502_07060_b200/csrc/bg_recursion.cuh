@@ -115,14 +115,15 @@ __device__ __forceinline__ void st_vec(typename F::E* p, const typename F::E (&v
     }
 }
 
-// sum_mu x_mu y_mu, plain (one operand already index-lowered), folded every kCap products
+// sum_mu x_mu y_mu, plain (one operand already index-lowered); headroom by F::relief (one operand
+// of every product is a canonical residue <= p-1: stored vectors always are)
 template <class F, int D>
 __device__ __forceinline__ typename F::A dot_plain(const typename F::E (&x)[D], const typename F::E (&y)[D])
 {
     typename F::A s = F::zero();
 #pragma unroll
     for (int mu = 0; mu < D; ++mu) {
-        if (mu && (mu % F::kCap) == 0) s = F::fold(s);
+        if (mu >= F::kCap0 && ((mu - F::kCap0) % F::kCapR) == 0) s = F::relief(s);
         s = F::mad(x[mu], y[mu], s);
     }
     return s;
@@ -136,7 +137,7 @@ __device__ __forceinline__ typename F::A dot_neg(typename F::E nx0, const typena
     typename F::A s = F::mad(nx0, y[0], F::zero());
 #pragma unroll
     for (int mu = 1; mu < D; ++mu) {
-        if ((mu % F::kCap) == 0) s = F::fold(s);
+        if (mu >= F::kCap0 && ((mu - F::kCap0) % F::kCapR) == 0) s = F::relief(s);
         s = F::mad(x[mu], y[mu], s);
     }
     return s;

@@ -86,7 +86,7 @@ __device__ __forceinline__ void tile_finish(typename F::E* __restrict__ rec, typ
     const E nhh = F::neg(F::mul(hsum, F::half()));               // -(sum_k h_k)/2
 #pragma unroll
     for (int mu = 0; mu < D; ++mu) {
-        acc[mu] = F::fold(acc[mu]);
+        acc[mu] = F::relief(acc[mu]);
         acc[mu] = F::mad(nhh, l[mu], acc[mu]);
         acc[mu] = F::mad(nhh, h[mu], acc[mu]);
     }
@@ -274,7 +274,7 @@ __global__ void __launch_bounds__(32 * W) bg_tile_kernel(const TileParams<typena
 #pragma unroll
                 for (int mu = 0; mu < D; ++mu) acc[mu] = F::zero();
                 hsum = F::ezero();
-                room = F::kCap;
+                room = F::kCap0;
             }
             if (fl & IT_LOAD_A) {
                 ld_vec<F, D>(reinterpret_cast<const E*>(recb + o.a), a);
@@ -293,18 +293,25 @@ __global__ void __launch_bounds__(32 * W) bg_tile_kernel(const TileParams<typena
                 const E cb = F::sub(xa, ua);
                 const E ca = F::sub(vb, xb);
                 hsum = F::add(hsum, h);
-                if (room < 3) {
+                if (room < 2) {
 #pragma unroll
-                    for (int mu = 0; mu < D; ++mu) acc[mu] = F::fold(acc[mu]);
-                    room = F::kCap;
+                    for (int mu = 0; mu < D; ++mu) acc[mu] = F::relief(acc[mu]);
+                    room = F::kCapR;
                 }
-                room -= 3;
+                room -= 2;
 #pragma unroll
                 for (int mu = 0; mu < D; ++mu) {
                     acc[mu] = F::mad(h, s[mu], acc[mu]);
                     acc[mu] = F::mad(cb, b[mu], acc[mu]);
-                    acc[mu] = F::mad(ca, a[mu], acc[mu]);
                 }
+                if (room < 1) {
+#pragma unroll
+                    for (int mu = 0; mu < D; ++mu) acc[mu] = F::relief(acc[mu]);
+                    room = F::kCapR;
+                }
+                room -= 1;
+#pragma unroll
+                for (int mu = 0; mu < D; ++mu) acc[mu] = F::mad(ca, a[mu], acc[mu]);
             } else {
                 // ---- 4-gluon split (i..k | k+1..l | l+1..j): 2 (A.C) J(k+1..l) ------------------------
                 E bm[D], c[D];
@@ -313,8 +320,8 @@ __global__ void __launch_bounds__(32 * W) bg_tile_kernel(const TileParams<typena
                 const E cc = F::neg(F::dbl(F::reduce(dot_neg<F, D>(na0, a, c))));   // 2 A.C
                 if (room < 1) {
 #pragma unroll
-                    for (int mu = 0; mu < D; ++mu) acc[mu] = F::fold(acc[mu]);
-                    room = F::kCap;
+                    for (int mu = 0; mu < D; ++mu) acc[mu] = F::relief(acc[mu]);
+                    room = F::kCapR;
                 }
                 room -= 1;
 #pragma unroll
