@@ -40,13 +40,16 @@ from paper_2502_07060_b200 import inputs  # noqa: E402
 
 METRIC = "amplitudes_per_second"
 UNIT = "amplitudes/s"
-# ALU-pipe bound of the canonical Mersenne-31 modular multiplication
-# (1 IMAD.WIDE on the FMA pipe + 3 ALU-pipe instructions; the ALU pipe issues 16 lanes per
-# clock per SM sub-partition = 64 per SM): 148 SMs x 64/3 per clock x max SM clock.
+# a field multiplication is one IMAD.WIDE.U32 (32x32(+64) -> 64); on sm_100 it
+# occupies the FMA-heavy pipe for 4 cycles per warp = 8 lanes per clock per SM sub-partition
+# = 32 per SM (measured by the register-resident probe bg_peaks.cu: 30.6; ncu: pipe_fmaheavy).
+# That pipe is the binding one for F_p, so the peak is 148 SMs x 32 per clock x max SM clock.
 SM_COUNT = 148
-ALU_LANES_PER_CLK_PER_SM = 64
-ALU_OPS_PER_MODMUL = 3
+WIDE_MUL_LANES_PER_CLK_PER_SM = 32
 DFMA_LANES_PER_CLK_PER_SM = 64      # checked against the DFMA probe
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the recursion kernel, from the committed
+# `ncu --set full` capture (profiles/r01b_cfg2_metrics.txt); algorithmic bytes are 407 MB
+NCU_TRAFFIC_BYTES = {"cfg2": 410.2e6}
 
 
 def log(*a):
@@ -266,24 +269,28 @@ def roofline(field: str, n: int, d: int, batch: int, kernel_ms: float, sm_max_mh
     oc = op_counts(field, n, d)
     clk = (sm_max_mhz or 1965.0) * 1e6
     if field == "fp31":
-        peak = SM_COUNT * ALU_LANES_PER_CLK_PER_SM / ALU_OPS_PER_MODMUL * clk          # modmul/s
+        peak = SM_COUNT * WIDE_MUL_LANES_PER_CLK_PER_SM * clk                            # field mul/s
         achieved = oc["mul_ref"] * batch / (kernel_ms * 1e-3)
-        unit, what = "Gmodmul/s", ("M_ref field multiplications of the literal Eq.(6) evaluation per amplitude "
-                                   "(SURVEY.md §8(d)) x points / kernel time; peak = ALU-pipe bound of the "
-                                   "canonical 4-instruction Mersenne-31 modmul at max SM clock (DESIGN.md §Roofline)")
+        unit, what = "Gmul/s", ("M_ref field multiplications of the literal Eq.(6) evaluation per amplitude "
+                                "(SURVEY.md §8(d)) x points / kernel time; peak = IMAD.WIDE.U32 issue rate "
+                                "(8 lanes/clk/SMSP, FMA-heavy pipe) at max SM clock (DESIGN.md §7)")
     else:
         peak = SM_COUNT * DFMA_LANES_PER_CLK_PER_SM * clk                                # DFMA/s
         achieved = 4 * oc["mul_ref"] * batch / (kernel_ms * 1e-3)
         unit, what = "GDFMA/s", ("4 DFMA per complex multiply-add x M_ref x points / kernel time; peak = "
                                  "FP64-pipe issue rate at max SM clock (DESIGN.md §Roofline)")
     r = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": unit, "frac": achieved / peak,
-         "traffic": traffic, "peak_source": "derived (DESIGN.md §Roofline); MEASURED_PEAKS.json has no ALU peak",
+         "traffic": traffic, "peak_source": "derived from unit counts and clock (DESIGN.md §7), confirmed by the on-box probe; MEASURED_PEAKS.json has no ALU peak",
          "what": what, "mul_ref_per_amplitude": oc["mul_ref"], "kernel_ms": kernel_ms,
          "hbm_frac": oc["bytes"] * batch / (kernel_ms * 1e-3) / 1e9 / hbm_peak()}
     if probes:
-        key = "modmul" if field == "fp31" else "dfma"
+        key = "imad_wide" if field == "fp31" else "dfma"
         r["probe_peak"] = probes[key]["ops_per_s"] / 1e9
         r["frac_of_probe"] = achieved / probes[key]["ops_per_s"]
+        if field == "fp31":
+            # north_star's line: canonical Mersenne-31 modular multiplications per second (R_mm, measured)
+            r["modmul_line_Gmodmul_s"] = probes["modmul"]["ops_per_s"] / 1e9
+            r["frac_of_modmul_line"] = achieved / probes["modmul"]["ops_per_s"]
     return r
 
 
@@ -367,7 +374,7 @@ def run_gpu(args) -> None:
             line["pipe_probes_Gops"] = {k: round(v["ops_per_s"] / 1e9, 1) for k, v in probes.items()
                                         if isinstance(v, dict)}
         line["roofline"] = roofline(cfg["field"], cfg["n"], cfg["d"], batch, kernel_ms, clocks.get("sm_max_mhz"),
-                                    probes, args.traffic)
+                                    probes, args.traffic if name == "cfg2" else None)
         if world == 1 and not args.headline_only:
             per = []
             for other in inputs.CONFIGS:
@@ -385,10 +392,13 @@ def run_gpu(args) -> None:
         if world == 1 and not args.no_cpu_baseline:
             cores = host_cores()
             sample = args.oracle_points or pick_oracle_sample(name, cores, 10.0)
-            t = time_oracle(name, sample, cores)[0]
-            line["cpu_baseline"] = {"value": sample / t, "unit": UNIT, "cores": cores, "kind": "oracle",
+            t1 = time_oracle(name, sample, cores)[0]
+            reps = max(1, min(64, int(10.0 / max(t1, 1e-3))))      # about 10 s of CPU work in total
+            ts = [t1] + (time_oracle(name, sample, cores, repeats=reps - 1) if reps > 1 else [])
+            t = sum(ts)
+            line["cpu_baseline"] = {"value": sample * len(ts) / t, "unit": UNIT, "cores": cores, "kind": "oracle",
                                     "sample": f"the first {sample} points of {name} (same seeded workload), "
-                                              f"{t:.1f} s on {cores} threads"}
+                                              f"{len(ts)} passes, {t:.1f} s on {cores} threads"}
         print(json.dumps(line))
     if dist is not None:
         dist.barrier()
@@ -409,7 +419,7 @@ def main():
     ap.add_argument("--headline-only", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-probes", action="store_true")
-    ap.add_argument("--traffic", type=float, default=None,
+    ap.add_argument("--traffic", type=float, default=NCU_TRAFFIC_BYTES.get("cfg2"),
                     help="dram bytes per launch of the recursion kernel from the committed ncu capture "
                          "(profiles/); reported as roofline.traffic")
     args = ap.parse_args()

@@ -122,7 +122,8 @@ int bg_op_count(int field, int n, int d, bg_opcount_t* out);
 
 /* Launch configuration the library would use for (field, n, d). */
 typedef struct {
-    int specialised;         /* 1: (n, d) compiled in; 0: runtime-n instance */
+    int specialised;         /* 0: runtime-n kernel; (n, d) compiled in: 1 table-driven tile kernel,
+                                2 level-unrolled kernel (the one a call would launch) */
     int threads_per_block;
     int points_per_block;
     int smem_bytes_per_block;

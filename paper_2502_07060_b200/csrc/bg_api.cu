@@ -7,6 +7,7 @@
 #include "../../include/bg.h"
 #include "bg_recursion.cuh"
 #include "bg_tile.cuh"
+#include "bg_level.cuh"
 #include <stdlib.h>
 
 namespace {
@@ -100,6 +101,7 @@ const void* pick(int n, int d, int* s)
 // ---- the compile-time (n, d) fast path: bg_sweep_kernel<F, N, D, W> ---------------------------
 struct SweepEntry {
     int field, n, d, w;
+    int kind;                // 0: bg_tile_kernel (table-driven loop), 1: bg_level_kernel (levels unrolled)
     const void* func;
     size_t smem;
 };
@@ -107,7 +109,14 @@ struct SweepEntry {
 template <class F, int N, int D, int W>
 SweepEntry sweep_entry(int field)
 {
-    return SweepEntry{field, N, D, W, reinterpret_cast<const void*>(&bg::bg_tile_kernel<F, N, D, W>),
+    return SweepEntry{field, N, D, W, 0, reinterpret_cast<const void*>(&bg::bg_tile_kernel<F, N, D, W>),
+                      bg::TileCfg<F, N, D, W>::SMEM_BYTES};
+}
+
+template <class F, int N, int D, int W>
+SweepEntry level_entry(int field)
+{
+    return SweepEntry{field, N, D, W, 1, reinterpret_cast<const void*>(&bg::bg_level_kernel<F, N, D, W>),
                       bg::TileCfg<F, N, D, W>::SMEM_BYTES};
 }
 
@@ -116,11 +125,19 @@ SweepEntry sweep_entry(int field)
 const SweepEntry* sweep_table(int* count)
 {
     static const SweepEntry table[] = {
+        // defaults (first entry of a shape), chosen by measurement on B200 (profiles/r01b_README.md)
+        level_entry<Fp31, 8, 6, 4>(BG_FIELD_FP31),
+        level_entry<Fp31, 4, 4, 1>(BG_FIELD_FP31),
+        sweep_entry<Fp31, 10, 8, 8>(BG_FIELD_FP31),
+        sweep_entry<Fp31, 12, 6, 8>(BG_FIELD_FP31),
+        level_entry<C128, 6, 4, 2>(BG_FIELD_C128),
+        // alternatives, selected with BG_KERNEL=tile|level and BG_SWEEP_W=<warps per tile>
         sweep_entry<Fp31, 8, 6, 4>(BG_FIELD_FP31),
         sweep_entry<Fp31, 8, 6, 8>(BG_FIELD_FP31),
         sweep_entry<Fp31, 4, 4, 1>(BG_FIELD_FP31),
-        sweep_entry<Fp31, 10, 8, 8>(BG_FIELD_FP31),
-        sweep_entry<Fp31, 12, 6, 8>(BG_FIELD_FP31),
+        level_entry<Fp31, 8, 6, 6>(BG_FIELD_FP31),
+        level_entry<Fp31, 10, 8, 4>(BG_FIELD_FP31),
+        level_entry<C128, 6, 4, 4>(BG_FIELD_C128),
         sweep_entry<C128, 6, 4, 4>(BG_FIELD_C128),
         sweep_entry<C128, 6, 4, 2>(BG_FIELD_C128),
     };
@@ -135,9 +152,12 @@ const SweepEntry* find_sweep(int field, int n, int d)
     const char* env = getenv("BG_SWEEP_W");
     const int want = env ? atoi(env) : 0;
     if (env && want == 0) return nullptr;            // BG_SWEEP_W=0: force the runtime-n kernel
+    const char* kenv = getenv("BG_KERNEL");          // "tile" / "level": restrict the kernel family
+    const int kind = !kenv ? -1 : (strcmp(kenv, "tile") == 0 ? 0 : strcmp(kenv, "level") == 0 ? 1 : -1);
     const SweepEntry* first = nullptr;
     for (int i = 0; i < count; ++i) {
         if (t[i].field != field || t[i].n != n || t[i].d != d) continue;
+        if (kind >= 0 && t[i].kind != kind) continue;
         if (t[i].smem > (size_t)kMaxSmemPerBlock) continue;
         if (!first) first = &t[i];
         if (t[i].w == want) return &t[i];
@@ -404,15 +424,26 @@ int bg_kernel_info(int field, int n, int d, bg_kernel_info_t* out)
     LaunchPlan plan;
     int rc = make_plan(field, n, d, &plan);
     if (rc != BG_OK) return rc;
-    out->specialised = plan.specialised;
-    out->threads_per_block = plan.threads;
-    out->points_per_block = plan.threads;
-    out->smem_bytes_per_block = plan.smem_bytes;
-    out->smem_bytes_per_point = plan.stride * plan.elem_bytes;
-    int bps = kSmemPerSm / (plan.smem_bytes + kSmemReservedPerBlock);
+    const void* func = plan.func;
+    if (const SweepEntry* e = find_sweep(field, n, d)) {
+        // the compile-time (n, d) fast path: one tile of 32 points per block, e->w warps
+        out->specialised = 1 + e->kind;          // 1: bg_tile_kernel, 2: bg_level_kernel
+        out->threads_per_block = 32 * e->w;
+        out->points_per_block = 32;
+        out->smem_bytes_per_block = (int)e->smem;
+        out->smem_bytes_per_point = (int)(e->smem / 32);
+        func = e->func;
+    } else {
+        out->specialised = 0;
+        out->threads_per_block = plan.threads;
+        out->points_per_block = plan.threads;
+        out->smem_bytes_per_block = plan.smem_bytes;
+        out->smem_bytes_per_point = plan.stride * plan.elem_bytes;
+    }
+    int bps = kSmemPerSm / (out->smem_bytes_per_block + kSmemReservedPerBlock);
     out->blocks_per_sm = bps > 32 ? 32 : bps;
     cudaFuncAttributes attr;
-    if (cudaFuncGetAttributes(&attr, plan.func) == cudaSuccess) {
+    if (cudaFuncGetAttributes(&attr, func) == cudaSuccess) {
         out->regs_per_thread = attr.numRegs;
     } else {
         cudaGetLastError();

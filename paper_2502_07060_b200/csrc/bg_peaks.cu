@@ -18,12 +18,6 @@ constexpr uint32_t kP = 0x7fffffffu;
 constexpr int CHAINS = 8;
 constexpr int UNROLL = 8;
 
-__device__ __forceinline__ uint64_t mad_wide(uint32_t a, uint32_t b, uint64_t c)
-{
-    uint64_t d;
-    asm volatile("mad.wide.u32 %0, %1, %2, %3;" : "=l"(d) : "r"(a), "r"(b), "l"(c));
-    return d;
-}
 __device__ __forceinline__ uint32_t mad_lo(uint32_t a, uint32_t b, uint32_t c)
 {
     uint32_t d;
@@ -61,15 +55,20 @@ __global__ void __launch_bounds__(256) peak_kernel(int iters, uint32_t seed, uin
 {
     const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
     if constexpr (KIND == BG_PEAK_IMAD_WIDE) {
+        // acc_c = lo(acc_{c+1}) * b + acc_c: the multiplicand comes from another chain, so the
+        // product can neither be hoisted nor strength-reduced; SASS is IMAD.WIDE.U32 R, R, R, R
+        // with a 64-bit addend (checked with cuobjdump; an inline-PTX mad.wide.u32 with a
+        // loop-invariant product is turned into plain adds and measures nothing).
         uint64_t acc[CHAINS];
-        uint32_t a = seed + t, b = (seed ^ 0x9e3779b9u) | 1u;
+        const uint32_t b = (seed ^ 0x9e3779b9u) | 1u;
 #pragma unroll
-        for (int c = 0; c < CHAINS; ++c) acc[c] = t + c;
+        for (int c = 0; c < CHAINS; ++c) acc[c] = ((const uint64_t*)sink)[(t * CHAINS + c) & 1023];
         for (int it = 0; it < iters; ++it) {
 #pragma unroll
             for (int u = 0; u < UNROLL; ++u)
 #pragma unroll
-                for (int c = 0; c < CHAINS; ++c) acc[c] = mad_wide(a, b, acc[c]);
+                for (int c = 0; c < CHAINS; ++c)
+                    acc[c] = (uint64_t)(uint32_t)acc[(c + 1) % CHAINS] * b + acc[c];
         }
         uint64_t s = 0;
 #pragma unroll
@@ -107,19 +106,22 @@ __global__ void __launch_bounds__(256) peak_kernel(int iters, uint32_t seed, uin
         for (int c = 0; c < CHAINS; ++c) s ^= acc[c];
         if (s == 0x12345678u) sink[t] = s;
     } else if constexpr (KIND == BG_PEAK_MIX) {
-        // one IMAD.WIDE + one ALU op per step on independent chains: do the pipes co-issue?
+        // one IMAD.WIDE (64-bit addend) + one ALU op per step on independent chains: do the pipes co-issue?
         uint64_t acc[CHAINS / 2];
         uint32_t alu[CHAINS / 2];
-        uint32_t a = seed + t, b = (seed ^ 0x9e3779b9u) | 1u;
+        const uint32_t a = seed + t, b = (seed ^ 0x9e3779b9u) | 1u;
 #pragma unroll
-        for (int c = 0; c < CHAINS / 2; ++c) { acc[c] = t + c; alu[c] = t ^ c; }
+        for (int c = 0; c < CHAINS / 2; ++c) {
+            acc[c] = ((const uint64_t*)sink)[(t * CHAINS + c) & 1023];
+            alu[c] = t ^ c;
+        }
         for (int it = 0; it < iters; ++it) {
 #pragma unroll
             for (int u = 0; u < UNROLL; ++u)
 #pragma unroll
                 for (int c = 0; c < CHAINS / 2; ++c) {
-                    acc[c] = mad_wide(a, b, acc[c]);
-                    alu[c] = (u & 1) ? add3(alu[c], a) : lop_xor_and(alu[c], a, 0x7fffffffu);
+                    acc[c] = (uint64_t)(uint32_t)acc[(c + 1) % (CHAINS / 2)] * b + acc[c];
+                    alu[c] = lop_xor_and(alu[c], a, 0x7fffffffu);
                 }
         }
         uint64_t s = 0;

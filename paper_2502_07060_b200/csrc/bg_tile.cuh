@@ -84,11 +84,20 @@ __device__ __forceinline__ void tile_finish(typename F::E* __restrict__ rec, typ
     ld_vec<F, D>(rec + (C::PS0 + lo) * D, l);
     ld_vec<F, D>(rec + (C::PS0 + hi) * D, h);
     const E nhh = F::neg(F::mul(hsum, F::half()));               // -(sum_k h_k)/2
+    if constexpr (F::kExact) {
+        // one product per component: the two ALU instructions of the add are cheaper than a
+        // second IMAD.WIDE (the multiplier pipe is the binding one)
 #pragma unroll
-    for (int mu = 0; mu < D; ++mu) {
-        acc[mu] = F::relief(acc[mu]);
-        acc[mu] = F::mad(nhh, l[mu], acc[mu]);
-        acc[mu] = F::mad(nhh, h[mu], acc[mu]);
+        for (int mu = 0; mu < D; ++mu) {
+            acc[mu] = F::relief(acc[mu]);
+            acc[mu] = F::mad(nhh, F::add(l[mu], h[mu]), acc[mu]);
+        }
+    } else {
+#pragma unroll
+        for (int mu = 0; mu < D; ++mu) {
+            acc[mu] = F::mad(nhh, l[mu], acc[mu]);
+            acc[mu] = F::mad(nhh, h[mu], acc[mu]);
+        }
     }
     E v[D];
     if (!top) {
@@ -120,27 +129,18 @@ __device__ __forceinline__ void tile_finish(typename F::E* __restrict__ rec, typ
     }
 }
 
+// a0-a3 for one tile: stage the inputs, doubled prefix sums, single-gluon U/V, invariants and
+// batch-inverted propagators.  Ends with a block barrier; shared by bg_tile_kernel and
+// bg_level_kernel (bg_level.cuh).
 template <class F, int N, int D, int W>
-__global__ void __launch_bounds__(32 * W) bg_tile_kernel(const TileParams<typename F::E> prm)
+__device__ __forceinline__ void tile_setup(typename F::E* __restrict__ vec, typename F::E* __restrict__ scal,
+                                           uint32_t* __restrict__ stat, const TileParams<typename F::E>& prm,
+                                           int lane, int warp, long long tile0, int valid, long long pt, bool live)
 {
     typedef TileCfg<F, N, D, W> C;
     typedef typename F::E E;
     typedef typename F::A A;
     constexpr int M = C::M, U = C::U, ND = N * D;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    E* vec = reinterpret_cast<E*>(smem_raw);                  // [32][VSTRIDE]
-    E* scal = vec + 32 * C::VSTRIDE;                          // [NSCAL][32]
-    uint32_t* stat = reinterpret_cast<uint32_t*>(scal + 32 * C::NSCAL);
-    const TileProgram<N, W>& tb = c_tile_program<F, N, D, W>;
-
-    // the warp index, broadcast from lane 0 so that everything derived from it (chunk bounds,
-    // item words, branch conditions) is compiled as warp-uniform
-    const int lane = threadIdx.x & 31, warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
-    const long long tile0 = (long long)blockIdx.x * 32;
-    const int valid = (int)min(32LL, prm.batch - tile0);
-    const long long pt = tile0 + lane;
-    const bool live = lane < valid;
-
     // ---- a0: stage the tile (coalesced, one vector unit per thread and step) ---------------------
     {
         typedef typename VecType<F, U>::type V;
@@ -245,6 +245,33 @@ __global__ void __launch_bounds__(32 * W) bg_tile_kernel(const TileParams<typena
     }
     __syncthreads();
     if (prm.status && warp == 0 && live) prm.status[pt] = stat[lane];
+
+}
+
+template <class F, int N, int D, int W>
+__global__ void __launch_bounds__(32 * W) bg_tile_kernel(const TileParams<typename F::E> prm)
+{
+    typedef TileCfg<F, N, D, W> C;
+    typedef typename F::E E;
+    typedef typename F::A A;
+    constexpr int M = C::M, U = C::U, ND = N * D;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    E* vec = reinterpret_cast<E*>(smem_raw);                  // [32][VSTRIDE]
+    E* scal = vec + 32 * C::VSTRIDE;                          // [NSCAL][32]
+    uint32_t* stat = reinterpret_cast<uint32_t*>(scal + 32 * C::NSCAL);
+    const TileProgram<N, W>& tb = c_tile_program<F, N, D, W>;
+
+    // the warp index, broadcast from lane 0 so that everything derived from it (chunk bounds,
+    // item words, branch conditions) is compiled as warp-uniform
+    const int lane = threadIdx.x & 31, warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
+    const long long tile0 = (long long)blockIdx.x * 32;
+    const int valid = (int)min(32LL, prm.batch - tile0);
+    const long long pt = tile0 + lane;
+    const bool live = lane < valid;
+
+    tile_setup<F, N, D, W>(vec, scal, stat, prm, lane, warp, tile0, valid, pt, live);
+    E* rec = vec + (size_t)lane * C::VSTRIDE;
+    E* sc = scal + lane;
 
     // ---- a4-a6: level sweep L = 2..m (Eq.(6)), amplitude, store ----------------------
 #pragma unroll 1
