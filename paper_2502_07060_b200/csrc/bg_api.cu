@@ -8,6 +8,7 @@
 #include "bg_recursion.cuh"
 #include "bg_tile.cuh"
 #include "bg_level.cuh"
+#include "bg_split.cuh"
 #include <stdlib.h>
 
 namespace {
@@ -101,7 +102,9 @@ const void* pick(int n, int d, int* s)
 // ---- the compile-time (n, d) fast path: bg_sweep_kernel<F, N, D, W> ---------------------------
 struct SweepEntry {
     int field, n, d, w;
-    int kind;                // 0: bg_tile_kernel (table-driven loop), 1: bg_level_kernel (levels unrolled)
+    int kind;                // 0: bg_tile_kernel (table-driven loop), 1: bg_level_kernel (levels unrolled),
+                             // 2: bg_split_kernel (table-driven, two lanes per point)
+    int tp;                  // points per tile (= per block)
     const void* func;
     size_t smem;
 };
@@ -109,15 +112,22 @@ struct SweepEntry {
 template <class F, int N, int D, int W>
 SweepEntry sweep_entry(int field)
 {
-    return SweepEntry{field, N, D, W, 0, reinterpret_cast<const void*>(&bg::bg_tile_kernel<F, N, D, W>),
+    return SweepEntry{field, N, D, W, 0, 32, reinterpret_cast<const void*>(&bg::bg_tile_kernel<F, N, D, W>),
                       bg::TileCfg<F, N, D, W>::SMEM_BYTES};
 }
 
 template <class F, int N, int D, int W>
 SweepEntry level_entry(int field)
 {
-    return SweepEntry{field, N, D, W, 1, reinterpret_cast<const void*>(&bg::bg_level_kernel<F, N, D, W>),
+    return SweepEntry{field, N, D, W, 1, 32, reinterpret_cast<const void*>(&bg::bg_level_kernel<F, N, D, W>),
                       bg::TileCfg<F, N, D, W>::SMEM_BYTES};
+}
+
+template <class F, int N, int D, int W>
+SweepEntry split_entry(int field)
+{
+    return SweepEntry{field, N, D, W, 2, 16, reinterpret_cast<const void*>(&bg::bg_split_kernel<F, N, D, W, 2>),
+                      bg::SplitCfg<F, N, D, W, 2>::SMEM_BYTES};
 }
 
 // first entry of a shape = the default warps-per-tile; the others can be selected with the
@@ -131,6 +141,7 @@ const SweepEntry* sweep_table(int* count)
         sweep_entry<Fp31, 10, 8, 8>(BG_FIELD_FP31),
         sweep_entry<Fp31, 12, 6, 8>(BG_FIELD_FP31),
         level_entry<C128, 6, 4, 2>(BG_FIELD_C128),
+        split_entry<C128, 12, 6, 8>(BG_FIELD_C128),
         // alternatives, selected with BG_KERNEL=tile|level and BG_SWEEP_W=<warps per tile>
         sweep_entry<Fp31, 8, 6, 4>(BG_FIELD_FP31),
         sweep_entry<Fp31, 8, 6, 8>(BG_FIELD_FP31),
@@ -140,6 +151,9 @@ const SweepEntry* sweep_table(int* count)
         level_entry<C128, 6, 4, 4>(BG_FIELD_C128),
         sweep_entry<C128, 6, 4, 4>(BG_FIELD_C128),
         sweep_entry<C128, 6, 4, 2>(BG_FIELD_C128),
+        split_entry<C128, 6, 4, 2>(BG_FIELD_C128),
+        split_entry<C128, 6, 4, 4>(BG_FIELD_C128),
+        split_entry<Fp31, 8, 6, 4>(BG_FIELD_FP31),
     };
     *count = (int)(sizeof(table) / sizeof(table[0]));
     return table;
@@ -153,7 +167,8 @@ const SweepEntry* find_sweep(int field, int n, int d)
     const int want = env ? atoi(env) : 0;
     if (env && want == 0) return nullptr;            // BG_SWEEP_W=0: force the runtime-n kernel
     const char* kenv = getenv("BG_KERNEL");          // "tile" / "level": restrict the kernel family
-    const int kind = !kenv ? -1 : (strcmp(kenv, "tile") == 0 ? 0 : strcmp(kenv, "level") == 0 ? 1 : -1);
+    const int kind = !kenv ? -1 : (strcmp(kenv, "tile") == 0 ? 0 : strcmp(kenv, "level") == 0 ? 1 :
+                                   strcmp(kenv, "split") == 0 ? 2 : -1);
     const SweepEntry* first = nullptr;
     for (int i = 0; i < count; ++i) {
         if (t[i].field != field || t[i].n != n || t[i].d != d) continue;
@@ -242,7 +257,7 @@ int launch_sweep(const SweepEntry& e, int64_t batch, const void* mom, const void
         cudaGetLastError();
         return BG_ERR_CUDA;
     }
-    const int64_t blocks = (batch + 31) / 32;
+    const int64_t blocks = (batch + e.tp - 1) / e.tp;
     if (blocks > 0x7fffffffLL) return BG_ERR_ARG;
     void* args[] = {&prm};
     if (cudaLaunchKernel(e.func, dim3((unsigned)blocks), dim3(32 * e.w), args, e.smem, stream) != cudaSuccess) {
@@ -427,11 +442,11 @@ int bg_kernel_info(int field, int n, int d, bg_kernel_info_t* out)
     const void* func = plan.func;
     if (const SweepEntry* e = find_sweep(field, n, d)) {
         // the compile-time (n, d) fast path: one tile of 32 points per block, e->w warps
-        out->specialised = 1 + e->kind;          // 1: bg_tile_kernel, 2: bg_level_kernel
+        out->specialised = 1 + e->kind;          // 1: bg_tile_kernel, 2: bg_level_kernel, 3: bg_split_kernel
         out->threads_per_block = 32 * e->w;
-        out->points_per_block = 32;
+        out->points_per_block = e->tp;
         out->smem_bytes_per_block = (int)e->smem;
-        out->smem_bytes_per_point = (int)(e->smem / 32);
+        out->smem_bytes_per_point = (int)(e->smem / e->tp);
         func = e->func;
     } else {
         out->specialised = 0;

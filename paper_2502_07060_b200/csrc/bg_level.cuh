@@ -44,7 +44,7 @@ struct LevelTask {
 struct LevelWeights {
     int w3, w4, wstart, wfin, wpart, wgather;
 };
-constexpr LevelWeights kLevelWeights = {80, 30, 25, 150, 40, 30};
+constexpr LevelWeights kLevelWeights = {95, 30, 50, 125, 60, 30};   // from the ncu source view, profiles/r01b
 
 template <int N, int W>
 struct LevelProgram {

@@ -60,7 +60,7 @@ def test_op_counts_match_the_survey_table(lib, n, d, field, mref, s3, s4, R, byt
 
 def test_kernel_info_and_bad_shapes(lib):
     ki = binding.bg_kernel_info(0, 8, 6)
-    assert ki["specialised"] >= 1 and ki["points_per_block"] == 32 and ki["threads_per_block"] % 32 == 0
+    assert ki["specialised"] >= 1 and ki["points_per_block"] in (16, 32) and ki["threads_per_block"] % 32 == 0
     assert ki["smem_bytes_per_block"] <= 232448
     assert binding.bg_kernel_info(0, 7, 6)["specialised"] == 0
     big = binding.bg_kernel_info(1, 16, 16)          # largest record: fewer points per block

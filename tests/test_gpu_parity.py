@@ -244,7 +244,9 @@ VARIANTS = [("fp31", 8, 6, "level", 4), ("fp31", 8, 6, "level", 6), ("fp31", 8, 
             ("fp31", 8, 6, "tile", 8), ("fp31", 4, 4, "level", 1), ("fp31", 4, 4, "tile", 1),
             ("fp31", 10, 8, "tile", 8), ("fp31", 10, 8, "level", 4), ("fp31", 12, 6, "tile", 8),
             ("c128", 6, 4, "level", 2), ("c128", 6, 4, "level", 4), ("c128", 6, 4, "tile", 4),
-            ("c128", 6, 4, "tile", 2), ("fp31", 8, 6, "general", 0), ("c128", 6, 4, "general", 0)]
+            ("c128", 6, 4, "tile", 2), ("fp31", 8, 6, "general", 0), ("c128", 6, 4, "general", 0),
+            ("c128", 12, 6, "split", 8), ("c128", 6, 4, "split", 2), ("c128", 6, 4, "split", 4),
+            ("fp31", 8, 6, "split", 4)]
 
 
 @pytest.mark.parametrize("field,n,d,kernel,w", VARIANTS, ids=lambda v: str(v))
@@ -263,8 +265,14 @@ def test_kernel_variants(bgl, oracle_mod, monkeypatch, field, n, d, kernel, w):
         assert np.array_equal(bgl.to_numpy(out), ref)
         assert np.array_equal(bgl.to_numpy(cur)[:, iu[0], iu[1]], rcur[:, iu[0], iu[1]])
     else:
-        mom, pol, _ = inputs.make_complex_inputs(n, d, batch, seed=31, helicities=(-1, -1, 1, 1, 1, 1))
+        mom, pol, _ = inputs.make_complex_inputs(n, d, batch, seed=31,
+                                                 helicities=(-1, -1, 1, 1, 1, 1) if n == 6 else None)
         dbl = oracle_mod.amplitudes(oracle_mod.C128, mom, pol, threads=8)
         truth = oracle_mod.amplitudes(oracle_mod.C80, mom, pol, threads=8)
         ok, e_g, _ = _complex_rule(_gpu_amplitudes(bgl, mom, pol), dbl, truth, _kappa(oracle_mod, mom, pol, dbl))
         assert ok.all() and np.median(e_g) < 1e-12
+        ref, rcur = oracle_mod.amplitudes(oracle_mod.C128, mom, pol, threads=8, want_currents=True)
+        out, cur, _ = bgl.currents(bgl.to_device(mom), bgl.to_device(pol))
+        iu = np.triu_indices(n - 1)
+        a, b = bgl.to_numpy(cur)[:, iu[0], iu[1]], rcur[:, iu[0], iu[1]]
+        assert np.all(np.abs(a - b) <= 1e-8 * (np.abs(b).max(axis=-1, keepdims=True)))
