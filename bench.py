@@ -370,9 +370,15 @@ def run_gpu(args) -> None:
     if rank == 0:
         probes = None
         if not args.no_probes:
-            probes = measure.measure_peaks(kinds=["imad_wide", "alu", "mix", "modmul", "dfma", "lds64"])
+            probes = measure.measure_peaks(kinds=["imad_wide", "alu", "mix", "mix2", "mix3", "modmul", "dfma", "lds64"])
             line["pipe_probes_Gops"] = {k: round(v["ops_per_s"] / 1e9, 1) for k, v in probes.items()
                                         if isinstance(v, dict)}
+            # SM sub-partition cycles per warp for one IMAD.WIDE (64-bit addend) + n ALU instructions:
+            # independent pipes would give max(4, 2n); measured is additive
+            smsp_hz = SM_COUNT * 4 * (clocks.get("sm_max_mhz") or 1965.0) * 1e6
+            line["wide_plus_n_alu_cycles"] = {
+                str(n): round(smsp_hz / (probes[k]["ops_per_s"] / (n + 1) / 32), 2)
+                for n, k in ((1, "mix"), (2, "mix2"), (3, "mix3"))}
         line["roofline"] = roofline(cfg["field"], cfg["n"], cfg["d"], batch, kernel_ms, clocks.get("sm_max_mhz"),
                                     probes, args.traffic if name == "cfg2" else None)
         if world == 1 and not args.headline_only:

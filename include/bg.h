@@ -148,7 +148,9 @@ typedef enum {
     BG_PEAK_DFMA = 5,        /* FP64 fused multiply-add: R_dfma */
     BG_PEAK_LDS32 = 6,       /* shared-memory loads, 4/8/16 bytes per lane */
     BG_PEAK_LDS64 = 7,
-    BG_PEAK_LDS128 = 8
+    BG_PEAK_LDS128 = 8,
+    BG_PEAK_MIX2 = 9,        /* one IMAD.WIDE + two ALU ops per step (counts all three) */
+    BG_PEAK_MIX3 = 10        /* one IMAD.WIDE + three ALU ops per step (counts all four) */
 } bg_peak_kind_t;
 int bg_peak_probe(int kind, int iters, int blocks, int threads, uint32_t* sink,
                   int64_t* ops_per_thread, cudaStream_t stream);

@@ -105,8 +105,11 @@ __global__ void __launch_bounds__(256) peak_kernel(int iters, uint32_t seed, uin
 #pragma unroll
         for (int c = 0; c < CHAINS; ++c) s ^= acc[c];
         if (s == 0x12345678u) sink[t] = s;
-    } else if constexpr (KIND == BG_PEAK_MIX) {
-        // one IMAD.WIDE (64-bit addend) + one ALU op per step on independent chains: do the pipes co-issue?
+    } else if constexpr (KIND == BG_PEAK_MIX || KIND == BG_PEAK_MIX2 || KIND == BG_PEAK_MIX3) {
+        // one IMAD.WIDE (64-bit addend) + NALU ALU ops per step on independent chains: do the pipes
+        // co-issue?  (Measured: no -- the cost is additive, about 3.2 + 2 NALU cycles per warp and
+        // step, where independent pipes would give max(4, 2 NALU).)
+        constexpr int NALU = KIND == BG_PEAK_MIX ? 1 : KIND == BG_PEAK_MIX2 ? 2 : 3;
         uint64_t acc[CHAINS / 2];
         uint32_t alu[CHAINS / 2];
         const uint32_t a = seed + t, b = (seed ^ 0x9e3779b9u) | 1u;
@@ -121,7 +124,8 @@ __global__ void __launch_bounds__(256) peak_kernel(int iters, uint32_t seed, uin
 #pragma unroll
                 for (int c = 0; c < CHAINS / 2; ++c) {
                     acc[c] = (uint64_t)(uint32_t)acc[(c + 1) % (CHAINS / 2)] * b + acc[c];
-                    alu[c] = lop_xor_and(alu[c], a, 0x7fffffffu);
+#pragma unroll
+                    for (int j = 0; j < NALU; ++j) alu[c] = lop_xor_and(alu[c], a + j, 0x7fffffffu);
                 }
         }
         uint64_t s = 0;
@@ -213,6 +217,8 @@ extern "C" int bg_peak_probe(int kind, int iters, int blocks, int threads, uint3
         case BG_PEAK_IMAD: rc = launch<BG_PEAK_IMAD>(iters, blocks, threads, sink, stream); break;
         case BG_PEAK_ALU: rc = launch<BG_PEAK_ALU>(iters, blocks, threads, sink, stream); break;
         case BG_PEAK_MIX: rc = launch<BG_PEAK_MIX>(iters, blocks, threads, sink, stream); break;
+        case BG_PEAK_MIX2: rc = launch<BG_PEAK_MIX2>(iters, blocks, threads, sink, stream); per_iter = per_iter * 3 / 2; break;
+        case BG_PEAK_MIX3: rc = launch<BG_PEAK_MIX3>(iters, blocks, threads, sink, stream); per_iter *= 2; break;
         case BG_PEAK_MODMUL: rc = launch<BG_PEAK_MODMUL>(iters, blocks, threads, sink, stream); break;
         case BG_PEAK_DFMA: rc = launch<BG_PEAK_DFMA>(iters, blocks, threads, sink, stream); break;
         case BG_PEAK_LDS32: rc = launch<BG_PEAK_LDS32>(iters, blocks, threads, sink, stream); per_iter /= 4; break;
