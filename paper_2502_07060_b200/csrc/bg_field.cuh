@@ -39,7 +39,7 @@ struct Fp31 {
 
     __device__ __forceinline__ static E load_input(uint32_t raw)
     {   // values >= p are reduced on load (bg.h); raw < 2^32 = 2p + 2
-        uint32_t r = (raw & kP) + (raw >> 31);
+        uint32_t r = min(raw, raw - kP);                          // two conditional subtractions
         return min(r, r - kP);
     }
     __device__ __forceinline__ static A zero() { return 0ull; }

@@ -121,28 +121,19 @@ __device__ __forceinline__ void split_finish(typename F::E* __restrict__ rec, ty
     }
 }
 
+// a0-a3 for one 16-point tile (stage, doubled prefix sums, single-gluon U/V, invariants, batch-inverted
+// propagators); ends with a block barrier.  Shared by bg_split_kernel and bg_level2_kernel.
 template <class F, int N, int D, int W, int S>
-__global__ void __launch_bounds__(32 * W) bg_split_kernel(const TileParams<typename F::E> prm)
+__device__ __forceinline__ void split_setup(typename F::E* __restrict__ vec, typename F::E* __restrict__ scal,
+                                            uint32_t* __restrict__ stat, const TileParams<typename F::E>& prm,
+                                            int warp, int point, int half, bool t0, long long tile0, int valid,
+                                            long long pt, bool live)
 {
     typedef TileCfg<F, N, D, W> C;
     typedef SplitCfg<F, N, D, W, S> SC;
     typedef typename F::E E;
     typedef typename F::A A;
     constexpr int M = C::M, U = C::U, ND = N * D, TP = SC::TP, DL = SC::DL;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    E* vec = reinterpret_cast<E*>(smem_raw);                  // [TP][VSTRIDE]
-    E* scal = vec + TP * C::VSTRIDE;                          // [NSCAL][TP]
-    uint32_t* stat = reinterpret_cast<uint32_t*>(scal + TP * C::NSCAL);
-    const TileProgram<N, W>& tb = c_split_program<F, N, D, W, S>;
-
-    const int lane = threadIdx.x & 31, warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
-    const int point = lane & (TP - 1), half = lane / TP;
-    const bool t0 = half == 0;                                 // this lane owns the time component
-    const long long tile0 = (long long)blockIdx.x * TP;
-    const int valid = (int)min((long long)TP, prm.batch - tile0);
-    const long long pt = tile0 + point;
-    const bool live = point < valid;
-
     // ---- a0: stage the tile (coalesced, one vector unit per thread and step) ---------------------
     {
         typedef typename VecType<F, U>::type V;
@@ -246,6 +237,34 @@ __global__ void __launch_bounds__(32 * W) bg_split_kernel(const TileParams<typen
     }
     __syncthreads();
     if (prm.status && warp == 0 && half == 0 && live) prm.status[pt] = stat[point];
+
+}
+
+template <class F, int N, int D, int W, int S>
+__global__ void __launch_bounds__(32 * W) bg_split_kernel(const TileParams<typename F::E> prm)
+{
+    typedef TileCfg<F, N, D, W> C;
+    typedef SplitCfg<F, N, D, W, S> SC;
+    typedef typename F::E E;
+    typedef typename F::A A;
+    constexpr int M = C::M, U = C::U, ND = N * D, TP = SC::TP, DL = SC::DL;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    E* vec = reinterpret_cast<E*>(smem_raw);                  // [TP][VSTRIDE]
+    E* scal = vec + TP * C::VSTRIDE;                          // [NSCAL][TP]
+    uint32_t* stat = reinterpret_cast<uint32_t*>(scal + TP * C::NSCAL);
+    const TileProgram<N, W>& tb = c_split_program<F, N, D, W, S>;
+
+    const int lane = threadIdx.x & 31, warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
+    const int point = lane & (TP - 1), half = lane / TP;
+    const bool t0 = half == 0;                                 // this lane owns the time component
+    const long long tile0 = (long long)blockIdx.x * TP;
+    const int valid = (int)min((long long)TP, prm.batch - tile0);
+    const long long pt = tile0 + point;
+    const bool live = point < valid;
+
+    split_setup<F, N, D, W, S>(vec, scal, stat, prm, warp, point, half, t0, tile0, valid, pt, live);
+    E* rec = vec + (size_t)point * C::VSTRIDE + half * DL;   // this lane's components of the point's record
+    E* sc = scal + point;
 
     // ---- a4-a6: level sweep L = 2..m (Eq.(6)), amplitude, store ----------------------
 #pragma unroll 1

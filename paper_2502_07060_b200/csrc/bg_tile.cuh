@@ -59,6 +59,23 @@ __constant__ TileProgram<N, W> c_tile_program = make_tile_program<N, W>(
     D * (int)sizeof(typename F::E), TileCfg<F, N, D, W>::PS0, TileCfg<F, N, D, W>::SC_U, TileCfg<F, N, D, W>::SC_V,
     32 * (int)sizeof(typename F::E));
 
+// proper multi-gluon range r (level-major) -> lo | hi << 8 with P_{i,j} = PS_hi - PS_lo
+template <int N>
+struct TileRanges {
+    uint16_t lohi[(N - 1) * (N - 2) / 2];
+};
+template <int N>
+constexpr TileRanges<N> make_tile_ranges()
+{
+    TileRanges<N> t{};
+    int r = 0;
+    for (int L = 2; L <= N - 2; ++L)
+        for (int i = 0; i + L <= N - 1; ++i) t.lohi[r++] = (uint16_t)(i | (i + L) << 8);
+    return t;
+}
+template <int N>
+__constant__ TileRanges<N> c_tile_ranges = make_tile_ranges<N>();
+
 template <class E>
 struct TileParams {
     const E* mom;         // [batch][n][D]
@@ -148,11 +165,12 @@ __device__ __forceinline__ void tile_setup(typename F::E* __restrict__ vec, type
         const V* gp = reinterpret_cast<const V*>(prm.pol + tile0 * ND);
         const V* gm = reinterpret_cast<const V*>(prm.mom + tile0 * ND);
         const int total = valid * UPP;
+#pragma unroll 4
         for (int g = threadIdx.x; g < total; g += 32 * W) {
             const int p = g / UPP, q = g - p * UPP;
             V* r = reinterpret_cast<V*>(vec + (size_t)p * C::VSTRIDE);
-            r[q] = load_unit<F>(gp[g]);
-            if (q < M * D / U) r[(C::PS0 + 1) * D / U + q] = load_unit<F>(gm[g]);         // k_n is never used
+            r[q] = load_unit<F>(__ldg(gp + g));
+            if (q < M * D / U) r[(C::PS0 + 1) * D / U + q] = load_unit<F>(__ldg(gm + g));  // k_n is never used
         }
         if (warp == 0) stat[lane] = 0;
     }
@@ -198,12 +216,11 @@ __device__ __forceinline__ void tile_setup(typename F::E* __restrict__ vec, type
         uint32_t status = 0;
 #pragma unroll 1
         for (int r = warp; r < C::R; r += W) {
-            // range r -> (L, i): level-major, level L has M-L+1 ranges
-            int L = 2, i = r;
-            while (i >= M - L + 1) { i -= M - L + 1; ++L; }
+            // range r -> (i, i+L) from the constant table: level-major, level L has M-L+1 ranges
+            const uint32_t rg = c_tile_ranges<N>.lohi[r];
             E lo[D], hi[D], x[D];
-            ld_vec<F, D>(rec + (C::PS0 + i) * D, lo);
-            ld_vec<F, D>(rec + (C::PS0 + i + L) * D, hi);
+            ld_vec<F, D>(rec + (C::PS0 + (rg & 255u)) * D, lo);
+            ld_vec<F, D>(rec + (C::PS0 + (rg >> 8)) * D, hi);
 #pragma unroll
             for (int mu = 0; mu < D; ++mu) x[mu] = F::sub(hi[mu], lo[mu]);
             const A ns = dot_neg<F, D>(F::neg(x[0]), x, x);                  // -(2P).(2P)
