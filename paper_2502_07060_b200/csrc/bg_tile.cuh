@@ -158,6 +158,7 @@ __device__ __forceinline__ void tile_setup(typename F::E* __restrict__ vec, type
     typedef typename F::E E;
     typedef typename F::A A;
     constexpr int M = C::M, U = C::U, ND = N * D;
+    constexpr bool kParPrefix = W > 1 && C::R >= M;          // room to park the momenta in the multi-gluon rows
     // ---- a0: stage the tile (coalesced, one vector unit per thread and step) ---------------------
     {
         typedef typename VecType<F, U>::type V;
@@ -170,7 +171,10 @@ __device__ __forceinline__ void tile_setup(typename F::E* __restrict__ vec, type
             const int p = g / UPP, q = g - p * UPP;
             V* r = reinterpret_cast<V*>(vec + (size_t)p * C::VSTRIDE);
             r[q] = load_unit<F>(__ldg(gp + g));
-            if (q < M * D / U) r[(C::PS0 + 1) * D / U + q] = load_unit<F>(__ldg(gm + g));  // k_n is never used
+            // k_n is never used.  With several warps the momenta are parked in the rows of the
+            // multi-gluon currents (free until the level sweep), so that the prefix sums below can
+            // be formed by all warps at once without overwriting their own input.
+            if (q < M * D / U) r[(kParPrefix ? N : C::PS0 + 1) * D / U + q] = load_unit<F>(__ldg(gm + g));
         }
         if (warp == 0) stat[lane] = 0;
     }
@@ -181,7 +185,40 @@ __device__ __forceinline__ void tile_setup(typename F::E* __restrict__ vec, type
 
     // ---- a1: doubled prefix sums PS2_c = 2 (k_1 + .. + k_c)  (Eq.(7)) and the
     //      single-gluon U = V = 2 k_i . eps_i  (zero for transverse states; kept for any input)
-    if (warp == 0) {
+    if constexpr (kParPrefix) {
+        // row c is formed by warp (c-1) mod W from the parked momenta (same left-to-right order
+        // of additions as the running sum, so the floating-point result is the same)
+        if (warp == 0) {
+            E z[D];
+#pragma unroll
+            for (int mu = 0; mu < D; ++mu) z[mu] = F::ezero();
+            st_vec<F, D>(rec + C::PS0 * D, z);
+        }
+#pragma unroll 1
+        for (int c = warp + 1; c <= M; c += W) {
+            E run[D], k[D], e[D];
+            ld_vec<F, D>(rec + N * D, run);
+#pragma unroll 1
+            for (int l = 2; l <= c; ++l) {
+                ld_vec<F, D>(rec + (N + l - 1) * D, k);
+#pragma unroll
+                for (int mu = 0; mu < D; ++mu) run[mu] = F::add(run[mu], k[mu]);
+            }
+            ld_vec<F, D>(rec + (N + c - 1) * D, k);
+            ld_vec<F, D>(rec + (c - 1) * D, e);
+#pragma unroll
+            for (int mu = 0; mu < D; ++mu) { k[mu] = F::dbl(k[mu]); run[mu] = F::dbl(run[mu]); }
+            const E u = F::neg(F::reduce(dot_neg<F, D>(F::neg(k[0]), k, e)));       // 2 k.eps
+            sc[(C::SC_U + c - 1) * 32] = u;
+            sc[(C::SC_V + c - 1) * 32] = u;
+            st_vec<F, D>(rec + (C::PS0 + c) * D, run);
+            if (prm.currents && live) {
+                E* dst = prm.currents + (pt * M * M + (long long)(c - 1) * M + (c - 1)) * D;
+#pragma unroll
+                for (int mu = 0; mu < D; ++mu) dst[mu] = F::canon(e[mu]);
+            }
+        }
+    } else if (warp == 0) {
         E run[D];
 #pragma unroll
         for (int mu = 0; mu < D; ++mu) run[mu] = F::ezero();
