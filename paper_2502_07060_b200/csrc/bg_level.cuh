@@ -60,28 +60,75 @@ constexpr LevelProgram<N, W> make_level_program(LevelWeights wt = kLevelWeights)
     LevelProgram<N, W> p{};
     constexpr int M = N - 1;
     constexpr int PER = M + W + 2;       // tasks per (level, warp) at most
+    constexpr int MAXCNT = (M / 2 + 1) * (M / 2 + 1);   // >= (L-1)(M-L+1) units of any level
     int nt = 0;
     for (int L = 0; L <= M; ++L)
         for (int w = 0; w <= W; ++w) p.beg[L][w] = 0;
     for (int L = 2; L <= M; ++L) {
         const int NU = L - 1, NC = M - L + 1, cnt = NU * NC;
-        // total weight
-        long total = 0;
-        for (int la = 1; la <= NU; ++la) total += wt.w3 + (long)(NU - la) * wt.w4;
-        total = (total + wt.wstart + wt.wfin) * NC;
-        // chunk boundaries in flattened unit index q = ci * NU + (la - 1)
+        // chunk boundaries in flattened unit index q = ci * NU + (la - 1): the contiguous partition
+        // into W chunks with the smallest modelled level time, found by dynamic programming over
+        // the cut positions (cost of a chunk = its units + start + finish or partial store of
+        // every current it touches); candidates with a penalty on shared currents are compared by
+        // the full model (largest chunk + largest gather load, as executed around the barrier).
         int cut[W + 1] = {};
         {
-            long cum = 0;
-            int w = 1;
-            for (int q = 0; q < cnt; ++q) {
-                const int u = q % NU;
-                while (w < W && cum * W >= (long)w * total) cut[w++] = q;
-                if (u == 0) cum += wt.wstart;
-                cum += wt.w3 + (long)(NU - 1 - u) * wt.w4;
-                if (u == NU - 1) cum += wt.wfin;
+            long pre[MAXCNT + 1] = {};
+            for (int q = 0; q < cnt; ++q) pre[q + 1] = pre[q] + wt.w3 + (long)(NU - 1 - q % NU) * wt.w4;
+            long best_time = -1;
+            for (int cand = 0; cand < 3; ++cand) {
+                const long pen = cand == 0 ? 0 : cand == 1 ? 100 : 100000;    // 100000: whole currents only
+                long bestv[W + 1][MAXCNT + 1] = {};
+                int arg[W + 1][MAXCNT + 1] = {};
+                for (int w = 0; w <= W; ++w)
+                    for (int q = 0; q <= cnt; ++q) bestv[w][q] = q == 0 && w == 0 ? 0 : (long)1 << 60;
+                for (int w = 1; w <= W; ++w)
+                    for (int q = 0; q <= cnt; ++q)
+                        for (int pp = 0; pp <= q; ++pp) {
+                            long c = 0;
+                            if (pp < q) {
+                                c = pre[q] - pre[pp];
+                                for (int ci = pp / NU; ci <= (q - 1) / NU; ++ci) {
+                                    const int lo = pp - ci * NU > 0 ? pp - ci * NU : 0;
+                                    const int hi = q - ci * NU < NU ? q - ci * NU : NU;
+                                    c += wt.wstart + (lo == 0 && hi == NU ? wt.wfin : wt.wpart + pen);
+                                }
+                            }
+                            const long v = bestv[w - 1][pp] > c ? bestv[w - 1][pp] : c;
+                            if (v < bestv[w][q]) { bestv[w][q] = v; arg[w][q] = pp; }
+                        }
+                int cc[W + 1] = {};
+                for (int w = W, q = cnt; w >= 1; --w) { cc[w] = q; q = arg[w][q]; }
+                // full model of this candidate
+                long la = 0, load[W] = {}, gl[W] = {};
+                int shared[MAXCNT + 1] = {};
+                for (int w = 0; w < W; ++w) {
+                    const int ub = cc[w], ue = cc[w + 1];
+                    if (ub >= ue) continue;
+                    load[w] = pre[ue] - pre[ub];
+                    for (int ci = ub / NU; ci <= (ue - 1) / NU; ++ci) {
+                        const int lo = ub - ci * NU > 0 ? ub - ci * NU : 0;
+                        const int hi = ue - ci * NU < NU ? ue - ci * NU : NU;
+                        const bool complete = lo == 0 && hi == NU;
+                        load[w] += wt.wstart + (complete ? wt.wfin : wt.wpart);
+                        if (!complete) ++shared[ci];
+                    }
+                    if (load[w] > la) la = load[w];
+                }
+                long lb = 0;
+                for (int ci = 0; ci < NC; ++ci)
+                    if (shared[ci]) {
+                        int b = 0;
+                        for (int w = 1; w < W; ++w)
+                            if (load[w] + gl[w] < load[b] + gl[b]) b = w;
+                        gl[b] += wt.wfin + (long)shared[ci] * wt.wgather;
+                        if (gl[b] > lb) lb = gl[b];
+                    }
+                if (best_time < 0 || la + lb < best_time) {
+                    best_time = la + lb;
+                    for (int w = 0; w <= W; ++w) cut[w] = cc[w];
+                }
             }
-            while (w <= W) cut[w++] = cnt;
         }
         LevelTask tmp[W][PER] = {};
         int ntw[W] = {};
