@@ -147,7 +147,6 @@ const SweepEntry* sweep_table(int* count)
         sweep_entry<Fp31, 8, 6, 8>(BG_FIELD_FP31),
         sweep_entry<Fp31, 4, 4, 1>(BG_FIELD_FP31),
         level_entry<Fp31, 8, 6, 6>(BG_FIELD_FP31),
-        level_entry<Fp31, 10, 8, 4>(BG_FIELD_FP31),
         level_entry<C128, 6, 4, 4>(BG_FIELD_C128),
         sweep_entry<C128, 6, 4, 4>(BG_FIELD_C128),
         sweep_entry<C128, 6, 4, 2>(BG_FIELD_C128),
