@@ -133,6 +133,12 @@ typedef struct {
 } bg_kernel_info_t;
 int bg_kernel_info(int field, int n, int d, bg_kernel_info_t* out);
 
+/* Host-side self-check of the compile-time work schedules of the tiled kernels (every splitting
+ * of Eq.(6), executed exactly once; parts of a shared current gathered exactly once;
+ * barriers taken by every warp).  Needs no GPU.  Returns 0, or a negative code naming the first
+ * violated rule. */
+int bg_selftest_schedules(void);
+
 /* ---- measurement support ---------------------------------------------------------------- */
 
 /* Register-resident issue-rate microbenchmarks (csrc/bg_peaks.cu): launches one kernel of

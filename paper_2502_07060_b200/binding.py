@@ -24,7 +24,7 @@ P31 = (1 << 31) - 1
 
 EXPORTS = ["bg_amplitudes", "bg_amplitudes_status", "bg_currents", "bg_amplitudes_host",
            "bg_host_workspace_bytes", "bg_modulus", "bg_status_string", "bg_version",
-           "bg_op_count", "bg_kernel_info", "bg_peak_probe"]
+           "bg_op_count", "bg_kernel_info", "bg_peak_probe", "bg_selftest_schedules"]
 
 
 class BgError(RuntimeError):
@@ -130,6 +130,10 @@ def bg_op_count(field, n, d) -> dict:
     oc = OpCount()
     _check(load().bg_op_count(field, n, d, ctypes.byref(oc)))
     return {k: int(getattr(oc, k)) for k, _ in OpCount._fields_}
+
+
+def bg_selftest_schedules() -> int:
+    return int(load().bg_selftest_schedules())
 
 
 def bg_kernel_info(field, n, d) -> dict:

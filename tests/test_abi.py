@@ -90,3 +90,8 @@ def test_product_does_not_import_the_oracle():
             src = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_2502_07060_b200" not in src and "from paper_2502_07060_b200" not in src, f
             assert not re.search(r'#\s*include\s*[<"][^">]*(bg\.h|\.cuh)', src), f
+
+
+def test_compile_time_schedules_are_valid(lib):
+    """every splitting of every current exactly once, parts gathered once, barriers by every warp"""
+    assert binding.bg_selftest_schedules() == 0
