@@ -13,7 +13,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libbg_b200.so")
 SOURCES = ["bg_api.cu", "bg_peaks.cu", "bg_selftest.cu"]
-HEADERS = ["bg_field.cuh", "bg_recursion.cuh", "bg_tables.cuh", "bg_tile.cuh", "bg_level.cuh", "bg_split.cuh"]
+HEADERS = ["bg_field.cuh", "bg_recursion.cuh", "bg_tables.cuh", "bg_tile.cuh", "bg_level.cuh", "bg_split.cuh", "bg_reg.cuh"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -9,6 +9,7 @@
 #include "bg_tile.cuh"
 #include "bg_level.cuh"
 #include "bg_split.cuh"
+#include "bg_reg.cuh"
 #include <stdlib.h>
 
 namespace {
@@ -102,7 +103,7 @@ const void* pick(int n, int d, int* s)
 // ---- the compile-time (n, d) fast path: bg_sweep_kernel<F, N, D, W> ---------------------------
 struct SweepEntry {
     int field, n, d, w;
-    int kind;                // 0: bg_tile_kernel (table-driven loop), 1: bg_level_kernel (levels unrolled),
+    int kind;                // 3: bg_reg_kernel (currents in registers, no barriers); 0: bg_tile_kernel (table-driven loop), 1: bg_level_kernel (levels unrolled),
                              // 2: bg_split_kernel (table-driven, two lanes per point)
     int tp;                  // points per tile (= per block)
     const void* func;
@@ -130,6 +131,14 @@ SweepEntry split_entry(int field)
                       bg::SplitCfg<F, N, D, W, 2>::SMEM_BYTES};
 }
 
+template <class F, int N, int D>
+SweepEntry reg_entry(int field)
+{
+    // kind 3: bg_reg_kernel; "w" = independent warps per block, 16 points per warp
+    return SweepEntry{field, N, D, bg::RegCfg<F, N, D>::WARPS, 3, 16 * bg::RegCfg<F, N, D>::WARPS,
+                      reinterpret_cast<const void*>(&bg::bg_reg_kernel<F, N, D>), bg::RegCfg<F, N, D>::SMEM_BYTES};
+}
+
 // first entry of a shape = the default warps-per-tile; the others can be selected with the
 // tuning knob BG_SWEEP_W (environment, read per call; used by the benchmarks' sweeps)
 const SweepEntry* sweep_table(int* count)
@@ -140,7 +149,7 @@ const SweepEntry* sweep_table(int* count)
         level_entry<Fp31, 4, 4, 1>(BG_FIELD_FP31),
         sweep_entry<Fp31, 10, 8, 8>(BG_FIELD_FP31),
         sweep_entry<Fp31, 12, 6, 8>(BG_FIELD_FP31),
-        level_entry<C128, 6, 4, 2>(BG_FIELD_C128),
+        reg_entry<C128, 6, 4>(BG_FIELD_C128),
         split_entry<C128, 12, 6, 8>(BG_FIELD_C128),
         // alternatives, selected with BG_KERNEL=tile|level and BG_SWEEP_W=<warps per tile>
         sweep_entry<Fp31, 8, 6, 4>(BG_FIELD_FP31),
@@ -151,6 +160,7 @@ const SweepEntry* sweep_table(int* count)
         sweep_entry<C128, 6, 4, 4>(BG_FIELD_C128),
         sweep_entry<C128, 6, 4, 2>(BG_FIELD_C128),
         split_entry<C128, 6, 4, 2>(BG_FIELD_C128),
+        level_entry<C128, 6, 4, 2>(BG_FIELD_C128),
         split_entry<C128, 6, 4, 4>(BG_FIELD_C128),
         split_entry<Fp31, 8, 6, 4>(BG_FIELD_FP31),
     };
@@ -167,7 +177,7 @@ const SweepEntry* find_sweep(int field, int n, int d)
     if (env && want == 0) return nullptr;            // BG_SWEEP_W=0: force the runtime-n kernel
     const char* kenv = getenv("BG_KERNEL");          // "tile" / "level": restrict the kernel family
     const int kind = !kenv ? -1 : (strcmp(kenv, "tile") == 0 ? 0 : strcmp(kenv, "level") == 0 ? 1 :
-                                   strcmp(kenv, "split") == 0 ? 2 : -1);
+                                   strcmp(kenv, "split") == 0 ? 2 : strcmp(kenv, "reg") == 0 ? 3 : -1);
     const SweepEntry* first = nullptr;
     for (int i = 0; i < count; ++i) {
         if (t[i].field != field || t[i].n != n || t[i].d != d) continue;
