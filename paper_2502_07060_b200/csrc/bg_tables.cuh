@@ -3,10 +3,11 @@
 // The sums over splittings of Eq.(6) are flattened, level by level, into a
 // list of ITEMS: for the current (i..j) of length L, in la-major order, the 3-gluon split
 // (i..k | k+1..j), k = i+la-1, followed by the 4-gluon splits (i..k | k+1..l | l+1..j),
-// l = k+lb.  The list of a level is cut into W contiguous chunks of (nearly) equal weight,
-// one per warp of the tile, so the warps of a block stay balanced whatever the number of
-// currents at that level.  A chunk boundary may fall inside a current; such a current gets
-// its partial sums combined by a "gather job" after a block barrier.
+// l = k+lb.  The list of a level is cut into W contiguous chunks, one per warp of the tile,
+// chosen by dynamic programming over a cost model of the level (pass 2 below), so the warps
+// of a block stay balanced whatever the number of currents at that level.  A chunk boundary
+// may fall inside a current (in front of a 3-gluon split); such a current gets its partial
+// sums combined by a "gather job" after a block barrier.
 //
 // Everything here is evaluated by the compiler (constexpr) and lands in constant memory:
 // the kernel reads it with warp-uniform indices, and its code is a short loop over items
@@ -25,7 +26,6 @@ constexpr uint32_t IT_SEG_END = 8u;     // last item of a segment
 constexpr uint32_t IT_COMPLETE = 16u;   // at SEG_END: the segment is the whole current -> finish inline
 constexpr uint32_t IT_TOP = 32u;        // the current is J(1..n-1): no propagator, amplitude
 
-constexpr int kWeight3 = 8, kWeight4 = 3, kWeightFinish = 10;
 
 struct TileItem {
     // x: a_row | b_row << 8 | c << 16 | flags << 24
@@ -90,8 +90,7 @@ constexpr TileTables<N, W> make_tile_tables()
         const int NC = M - L + 1;
         const int per = (L - 1) + (L - 1) * (L - 2) / 2;       // items per current
         const int cnt = NC * per;
-        // pass 1: fill items (without flags), total weight
-        long total = 0;
+        // pass 1: fill items (without flags)
         {
             int idx = base;
             for (int i = 1; i <= NC; ++i)
@@ -102,33 +101,85 @@ constexpr TileTables<N, W> make_tile_tables()
                     t.items[idx].x = a | (uint32_t)tt_row(N, i + la, L - la) << 8 | (uint32_t)(i + la - 1) << 16;
                     t.items[idx].y = y;
                     ++idx;
-                    total += kWeight3;
                     for (int lb = 1; lb <= L - la - 1; ++lb) {
                         t.items[idx].x = a | (uint32_t)tt_row(N, i + la, lb) << 8 |
                                          (uint32_t)tt_row(N, i + la + lb, L - la - lb) << 16 | IT_KIND4 << 24;
                         t.items[idx].y = y;
                         ++idx;
-                        total += kWeight4;
                     }
                 }
-            total += (long)NC * kWeightFinish;
         }
-        // pass 2: chunk boundaries by cumulative weight
+        // pass 2: chunk boundaries.  Cuts are allowed in front of every 3-gluon split (the start of a
+        // group of items that share the left factor); the contiguous partition into W chunks with
+        // the smallest modelled level time is found by dynamic programming over the cut positions
+        // (chunk cost = its items + start + finish or partial store of every current it touches, in
+        // executed instructions), once freely and once with shared currents forbidden; the two are
+        // compared by the full model (largest chunk + largest gather load, gather job j on warp j mod W).
         {
-            long cum = 0;
-            int w = 1;
-            t.beg[L][0] = (uint16_t)base;
-            for (int q = 0; q < cnt; ++q) {
-                while (w < W && cum * W >= (long)w * total) {
-                    t.beg[L][w] = (uint16_t)(base + q);
-                    ++w;
-                }
-                cum += (t.items[base + q].x >> 24 & IT_KIND4) ? kWeight4 : kWeight3;
-                if ((q + 1) % per == 0) cum += kWeightFinish;
+            constexpr int kI3 = 105, kI4 = 55, kStart = 35, kFin = 160, kPart = 70, kGather = 30;
+            constexpr int MAXP = (M / 2 + 1) * (M / 2 + 1) + 2;
+            int pos[MAXP] = {};
+            int np = 0;
+            for (int q = 0; q < cnt; ++q)
+                if (!(t.items[base + q].x >> 24 & IT_KIND4)) pos[np++] = q;
+            pos[np++] = cnt;
+            long pre[MAXP] = {};                               // cost of the items before position k
+            for (int k = 0; k + 1 < np; ++k) {
+                long c = 0;
+                for (int q = pos[k]; q < pos[k + 1]; ++q) c += (t.items[base + q].x >> 24 & IT_KIND4) ? kI4 : kI3;
+                pre[k + 1] = pre[k] + c;
             }
-            while (w <= W) {
-                t.beg[L][w] = (uint16_t)(base + cnt);
-                ++w;
+            long best_time = -1;
+            for (int cand = 0; cand < 2; ++cand) {
+                const long pen = cand == 0 ? 0 : 1000000;
+                long bestv[W + 1][MAXP] = {};
+                int arg[W + 1][MAXP] = {};
+                for (int w = 0; w <= W; ++w)
+                    for (int k = 0; k < np; ++k) bestv[w][k] = (w == 0 && k == 0) ? 0 : (long)1 << 60;
+                for (int w = 1; w <= W; ++w)
+                    for (int k = 0; k < np; ++k)
+                        for (int pk = 0; pk <= k; ++pk) {
+                            if (bestv[w - 1][pk] >= bestv[w][k]) continue;
+                            long c = 0;
+                            if (pk < k) {
+                                const int pq = pos[pk], qq = pos[k];
+                                c = pre[k] - pre[pk];
+                                for (int cur = pq / per; cur <= (qq - 1) / per; ++cur) {
+                                    const bool whole = pq <= cur * per && qq >= (cur + 1) * per;
+                                    c += kStart + (whole ? kFin : kPart + pen);
+                                }
+                            }
+                            const long v = bestv[w - 1][pk] > c ? bestv[w - 1][pk] : c;
+                            if (v < bestv[w][k]) { bestv[w][k] = v; arg[w][k] = pk; }
+                        }
+                int cc[W + 1] = {};
+                for (int w = W, k = np - 1; w >= 1; --w) { cc[w] = pos[k]; k = arg[w][k]; }
+                // full model
+                long la = 0, lb = 0, gl[W] = {};
+                int shared_parts[M + 1] = {};
+                for (int w = 0; w < W; ++w) {
+                    const int pq = cc[w], qq = cc[w + 1];
+                    if (pq >= qq) continue;
+                    long c = 0;
+                    for (int q = pq; q < qq; ++q) c += (t.items[base + q].x >> 24 & IT_KIND4) ? kI4 : kI3;
+                    for (int cur = pq / per; cur <= (qq - 1) / per; ++cur) {
+                        const bool whole = pq <= cur * per && qq >= (cur + 1) * per;
+                        c += kStart + (whole ? kFin : kPart);
+                        if (!whole) ++shared_parts[cur];
+                    }
+                    if (c > la) la = c;
+                }
+                int nj = 0;
+                for (int cur = 0; cur < NC; ++cur)
+                    if (shared_parts[cur]) {
+                        gl[nj % W] += kFin + (long)shared_parts[cur] * kGather;
+                        if (gl[nj % W] > lb) lb = gl[nj % W];
+                        ++nj;
+                    }
+                if (nj <= W && (best_time < 0 || la + lb < best_time)) {
+                    best_time = la + lb;
+                    for (int w = 0; w <= W; ++w) t.beg[L][w] = (uint16_t)(base + cc[w]);
+                }
             }
         }
         // pass 3: flags, slots, gather jobs
