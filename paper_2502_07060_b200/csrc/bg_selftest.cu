@@ -158,5 +158,6 @@ extern "C" int bg_selftest_schedules(void)
     if ((rc = check_tile_tables<6, 4>())) return rc - 160000;
     if ((rc = check_tile_tables<6, 2>())) return rc - 170000;
     if ((rc = check_tile_tables<16, 8>())) return rc - 180000;
+    if ((rc = check_tile_tables<12, 16>())) return rc - 190000;
     return rc;
 }
