@@ -148,7 +148,7 @@ const SweepEntry* sweep_table(int* count)
         level_entry<Fp31, 8, 6, 4>(BG_FIELD_FP31),
         level_entry<Fp31, 4, 4, 1>(BG_FIELD_FP31),
         sweep_entry<Fp31, 10, 8, 8>(BG_FIELD_FP31),
-        sweep_entry<Fp31, 12, 6, 8>(BG_FIELD_FP31),
+        sweep_entry<Fp31, 12, 6, 16>(BG_FIELD_FP31),
         reg_entry<C128, 6, 4>(BG_FIELD_C128),
         split_entry<C128, 12, 6, 16>(BG_FIELD_C128),
         // alternatives, selected with BG_KERNEL=tile|level and BG_SWEEP_W=<warps per tile>
