@@ -6,10 +6,8 @@
 
 #include "../../include/bg.h"
 #include "bg_recursion.cuh"
-#include "bg_tile.cuh"
-#include "bg_level.cuh"
-#include "bg_split.cuh"
-#include "bg_reg.cuh"
+#include "bg_tile.cuh"      // TileParams
+#include "bg_entries.h"
 #include <stdlib.h>
 
 namespace {
@@ -100,91 +98,31 @@ const void* pick(int n, int d, int* s)
     return nullptr;
 }
 
-// ---- the compile-time (n, d) fast path: bg_sweep_kernel<F, N, D, W> ---------------------------
-struct SweepEntry {
-    int field, n, d, w;
-    int kind;                // 3: bg_reg_kernel (currents in registers, no barriers); 0: bg_tile_kernel (table-driven loop), 1: bg_level_kernel (levels unrolled),
-                             // 2: bg_split_kernel (table-driven, two lanes per point)
-    int tp;                  // points per tile (= per block)
-    const void* func;
-    size_t smem;
-};
-
-template <class F, int N, int D, int W>
-SweepEntry sweep_entry(int field)
-{
-    return SweepEntry{field, N, D, W, 0, 32, reinterpret_cast<const void*>(&bg::bg_tile_kernel<F, N, D, W>),
-                      bg::TileCfg<F, N, D, W>::SMEM_BYTES};
-}
-
-template <class F, int N, int D, int W>
-SweepEntry level_entry(int field)
-{
-    return SweepEntry{field, N, D, W, 1, 32, reinterpret_cast<const void*>(&bg::bg_level_kernel<F, N, D, W>),
-                      bg::TileCfg<F, N, D, W>::SMEM_BYTES};
-}
-
-template <class F, int N, int D, int W>
-SweepEntry split_entry(int field)
-{
-    return SweepEntry{field, N, D, W, 2, 16, reinterpret_cast<const void*>(&bg::bg_split_kernel<F, N, D, W, 2>),
-                      bg::SplitCfg<F, N, D, W, 2>::SMEM_BYTES};
-}
-
-template <class F, int N, int D>
-SweepEntry reg_entry(int field)
-{
-    // kind 3: bg_reg_kernel; "w" = independent warps per block, 16 points per warp
-    return SweepEntry{field, N, D, bg::RegCfg<F, N, D>::WARPS, 3, 16 * bg::RegCfg<F, N, D>::WARPS,
-                      reinterpret_cast<const void*>(&bg::bg_reg_kernel<F, N, D>), bg::RegCfg<F, N, D>::SMEM_BYTES};
-}
-
-// first entry of a shape = the default warps-per-tile; the others can be selected with the
-// tuning knob BG_SWEEP_W (environment, read per call; used by the benchmarks' sweeps)
-const SweepEntry* sweep_table(int* count)
-{
-    static const SweepEntry table[] = {
-        // defaults (first entry of a shape), chosen by measurement on B200 (profiles/r01b_README.md)
-        level_entry<Fp31, 8, 6, 4>(BG_FIELD_FP31),
-        level_entry<Fp31, 4, 4, 1>(BG_FIELD_FP31),
-        sweep_entry<Fp31, 10, 8, 8>(BG_FIELD_FP31),
-        sweep_entry<Fp31, 12, 6, 16>(BG_FIELD_FP31),
-        reg_entry<C128, 6, 4>(BG_FIELD_C128),
-        split_entry<C128, 12, 6, 16>(BG_FIELD_C128),
-        // alternatives, selected with BG_KERNEL=tile|level and BG_SWEEP_W=<warps per tile>
-        sweep_entry<Fp31, 8, 6, 4>(BG_FIELD_FP31),
-        sweep_entry<Fp31, 8, 6, 8>(BG_FIELD_FP31),
-        sweep_entry<Fp31, 4, 4, 1>(BG_FIELD_FP31),
-        level_entry<Fp31, 8, 6, 6>(BG_FIELD_FP31),
-        level_entry<C128, 6, 4, 4>(BG_FIELD_C128),
-        sweep_entry<C128, 6, 4, 4>(BG_FIELD_C128),
-        sweep_entry<C128, 6, 4, 2>(BG_FIELD_C128),
-        split_entry<C128, 6, 4, 2>(BG_FIELD_C128),
-        level_entry<C128, 6, 4, 2>(BG_FIELD_C128),
-        split_entry<C128, 6, 4, 4>(BG_FIELD_C128),
-        split_entry<Fp31, 8, 6, 4>(BG_FIELD_FP31),
-    };
-    *count = (int)(sizeof(table) / sizeof(table[0]));
-    return table;
-}
-
+// ---- the compile-time (n, d) fast path -------------------------------------------------------------
+// The instances live in three translation units (bg_inst_*.cu): the work lists of a kernel
+// instance sit in constant memory, and one module has 64 KB of it.
 const SweepEntry* find_sweep(int field, int n, int d)
 {
-    int count = 0;
-    const SweepEntry* t = sweep_table(&count);
     const char* env = getenv("BG_SWEEP_W");
     const int want = env ? atoi(env) : 0;
     if (env && want == 0) return nullptr;            // BG_SWEEP_W=0: force the runtime-n kernel
-    const char* kenv = getenv("BG_KERNEL");          // "tile" / "level": restrict the kernel family
-    const int kind = !kenv ? -1 : (strcmp(kenv, "tile") == 0 ? 0 : strcmp(kenv, "level") == 0 ? 1 :
-                                   strcmp(kenv, "split") == 0 ? 2 : strcmp(kenv, "reg") == 0 ? 3 : -1);
+    const char* kenv = getenv("BG_KERNEL");          // restrict the kernel family (A/B runs)
+    const int kind = !kenv ? -1 : strcmp(kenv, "tile") == 0 ? 0 : strcmp(kenv, "level") == 0 ? 1 :
+                                  strcmp(kenv, "split") == 0 ? 2 : strcmp(kenv, "reg") == 0 ? 3 :
+                                  strcmp(kenv, "unit") == 0 ? 4 : -1;
+    typedef const SweepEntry* (*TableFn)(int*);
+    static const TableFn tables[] = {bg_entries_default, bg_entries_fp_alt, bg_entries_c128_alt};
     const SweepEntry* first = nullptr;
-    for (int i = 0; i < count; ++i) {
-        if (t[i].field != field || t[i].n != n || t[i].d != d) continue;
-        if (kind >= 0 && t[i].kind != kind) continue;
-        if (t[i].smem > (size_t)kMaxSmemPerBlock) continue;
-        if (!first) first = &t[i];
-        if (t[i].w == want) return &t[i];
+    for (TableFn fn : tables) {
+        int count = 0;
+        const SweepEntry* t = fn(&count);
+        for (int i = 0; i < count; ++i) {
+            if (t[i].field != field || t[i].n != n || t[i].d != d) continue;
+            if (kind >= 0 && t[i].kind != kind) continue;
+            if (t[i].smem > (size_t)kMaxSmemPerBlock) continue;
+            if (!first) first = &t[i];
+            if (t[i].w == want) return &t[i];
+        }
     }
     return first;
 }

@@ -57,6 +57,7 @@ struct LevelProgram {
 template <int N, int W>
 constexpr LevelProgram<N, W> make_level_program(LevelWeights wt = kLevelWeights)
 {
+    static_assert(2 * W <= 16 && N <= 16, "slot, ci, lo, hi are 4-bit fields of a task word");
     LevelProgram<N, W> p{};
     constexpr int M = N - 1;
     constexpr int PER = M + W + 2;       // tasks per (level, warp) at most

@@ -241,12 +241,13 @@ def test_full_size_complex_sampled(bgl, oracle_mod, name):
 
 # ---- every compiled kernel family / warps-per-tile variant (selection knobs BG_KERNEL, BG_SWEEP_W) ---
 VARIANTS = [("fp31", 8, 6, "level", 4), ("fp31", 8, 6, "level", 6), ("fp31", 8, 6, "tile", 4),
-            ("fp31", 8, 6, "tile", 8), ("fp31", 4, 4, "level", 1), ("fp31", 4, 4, "tile", 1),
+            ("fp31", 4, 4, "level", 1), ("fp31", 4, 4, "tile", 1),
             ("fp31", 10, 8, "tile", 8), ("fp31", 12, 6, "tile", 16),
             ("c128", 6, 4, "level", 2), ("c128", 6, 4, "level", 4), ("c128", 6, 4, "tile", 4),
             ("c128", 6, 4, "tile", 2), ("fp31", 8, 6, "general", 0), ("c128", 6, 4, "general", 0),
             ("c128", 12, 6, "split", 16), ("c128", 6, 4, "split", 2), ("c128", 6, 4, "split", 4),
-            ("fp31", 8, 6, "split", 4), ("c128", 6, 4, "reg", 4)]
+            ("c128", 6, 4, "reg", 4), ("fp31", 8, 6, "unit", 4),
+            ("fp31", 10, 8, "unit", 8), ("fp31", 12, 6, "unit", 8)]
 
 
 @pytest.mark.parametrize("field,n,d,kernel,w", VARIANTS, ids=lambda v: str(v))
