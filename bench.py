@@ -284,7 +284,7 @@ def roofline(field: str, n: int, d: int, batch: int, kernel_ms: float, sm_max_mh
          "what": what, "mul_ref_per_amplitude": oc["mul_ref"], "kernel_ms": kernel_ms,
          "hbm_frac": oc["bytes"] * batch / (kernel_ms * 1e-3) / 1e9 / hbm_peak()}
     if probes:
-        key = "imad_wide" if field == "fp31" else "dfma"
+        key = "imad_wide_rz" if field == "fp31" else "dfma"       # the bare multiplier rate / the DFMA rate
         r["probe_peak"] = probes[key]["ops_per_s"] / 1e9
         r["frac_of_probe"] = achieved / probes[key]["ops_per_s"]
         if field == "fp31":
@@ -370,7 +370,7 @@ def run_gpu(args) -> None:
     if rank == 0:
         probes = None
         if not args.no_probes:
-            probes = measure.measure_peaks(kinds=["imad_wide", "alu", "mix", "mix2", "mix3", "modmul", "dfma", "lds64"])
+            probes = measure.measure_peaks(kinds=["imad_wide", "imad_wide_rz", "alu", "mix", "mix2", "mix3", "modmul", "dfma", "lds64"])
             line["pipe_probes_Gops"] = {k: round(v["ops_per_s"] / 1e9, 1) for k, v in probes.items()
                                         if isinstance(v, dict)}
             # SM sub-partition cycles per warp for one IMAD.WIDE (64-bit addend) + n ALU instructions:

@@ -156,7 +156,8 @@ typedef enum {
     BG_PEAK_LDS64 = 7,
     BG_PEAK_LDS128 = 8,
     BG_PEAK_MIX2 = 9,        /* one IMAD.WIDE + two ALU ops per step (counts all three) */
-    BG_PEAK_MIX3 = 10        /* one IMAD.WIDE + three ALU ops per step (counts all four) */
+    BG_PEAK_MIX3 = 10,       /* one IMAD.WIDE + three ALU ops per step (counts all four) */
+    BG_PEAK_IMAD_WIDE_RZ = 11 /* IMAD.WIDE.U32 without addend (32x32 -> 64): the bare multiplier rate */
 } bg_peak_kind_t;
 int bg_peak_probe(int kind, int iters, int blocks, int threads, uint32_t* sink,
                   int64_t* ops_per_thread, cudaStream_t stream);

@@ -19,7 +19,7 @@ from . import build as _build
 FIELD_FP31, FIELD_C128 = 0, 1
 BG_OK, BG_ERR_ARG, BG_ERR_UNSUPPORTED, BG_ERR_CUDA = 0, -1, -2, -3
 PEAK_KINDS = {"imad_wide": 0, "imad": 1, "alu": 2, "mix": 3, "modmul": 4, "dfma": 5,
-              "lds32": 6, "lds64": 7, "lds128": 8, "mix2": 9, "mix3": 10}
+              "lds32": 6, "lds64": 7, "lds128": 8, "mix2": 9, "mix3": 10, "imad_wide_rz": 11}
 P31 = (1 << 31) - 1
 
 EXPORTS = ["bg_amplitudes", "bg_amplitudes_status", "bg_currents", "bg_amplitudes_host",

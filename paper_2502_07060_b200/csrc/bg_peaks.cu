@@ -74,6 +74,21 @@ __global__ void __launch_bounds__(256) peak_kernel(int iters, uint32_t seed, uin
 #pragma unroll
         for (int c = 0; c < CHAINS; ++c) s ^= acc[c];
         if (s == 0x123456789abcdefull) sink[t] = (uint32_t)s;
+    } else if constexpr (KIND == BG_PEAK_IMAD_WIDE_RZ) {
+        // acc = hi(acc) * lo(acc): IMAD.WIDE.U32 R, R, R, RZ -- the bare 32x32 -> 64 multiplier rate
+        uint64_t acc[CHAINS];
+#pragma unroll
+        for (int c = 0; c < CHAINS; ++c) acc[c] = ((const uint64_t*)sink)[(t * CHAINS + c) & 1023] | 0x300000005ull;
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int u = 0; u < UNROLL; ++u)
+#pragma unroll
+                for (int c = 0; c < CHAINS; ++c) acc[c] = (uint64_t)(uint32_t)(acc[c] >> 32) * (uint32_t)acc[c];
+        }
+        uint64_t s = 0;
+#pragma unroll
+        for (int c = 0; c < CHAINS; ++c) s ^= acc[c];
+        if (s == 0x123456789abcdefull) sink[t] = (uint32_t)s;
     } else if constexpr (KIND == BG_PEAK_IMAD) {
         uint32_t acc[CHAINS];
         uint32_t a = seed + t, b = (seed ^ 0x9e3779b9u) | 1u;
@@ -214,6 +229,7 @@ extern "C" int bg_peak_probe(int kind, int iters, int blocks, int threads, uint3
     int rc;
     switch (kind) {
         case BG_PEAK_IMAD_WIDE: rc = launch<BG_PEAK_IMAD_WIDE>(iters, blocks, threads, sink, stream); break;
+        case BG_PEAK_IMAD_WIDE_RZ: rc = launch<BG_PEAK_IMAD_WIDE_RZ>(iters, blocks, threads, sink, stream); break;
         case BG_PEAK_IMAD: rc = launch<BG_PEAK_IMAD>(iters, blocks, threads, sink, stream); break;
         case BG_PEAK_ALU: rc = launch<BG_PEAK_ALU>(iters, blocks, threads, sink, stream); break;
         case BG_PEAK_MIX: rc = launch<BG_PEAK_MIX>(iters, blocks, threads, sink, stream); break;
