@@ -9,7 +9,7 @@ const SweepEntry* bg_entries_fp_alt(int* count)
         level_entry<Fp31, 8, 6, 6>(BG_FIELD_FP31),
         unit_entry<Fp31, 8, 6, 4>(BG_FIELD_FP31),
         sweep_entry<Fp31, 10, 8, 8>(BG_FIELD_FP31),
-        unit_entry<Fp31, 12, 6, 8>(BG_FIELD_FP31),
+        sweep_entry<Fp31, 12, 6, 16>(BG_FIELD_FP31),
     };
     *count = (int)(sizeof(table) / sizeof(table[0]));
     return table;

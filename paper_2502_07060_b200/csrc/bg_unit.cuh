@@ -20,13 +20,15 @@
 
 namespace bg {
 
-// element offsets of the operands of unit (L, la), relative to the current's base pointers
-// ri = rec + ci*D (vector rows) and si = sc + ci*32 (scalar tables)
+// BYTE offsets of the operands of unit (L, la), relative to the current's base pointers
+// ri = rec + ci*D (vector rows) and si = sc + ci*32 (scalar tables): ready for [register + uniform
+// register + immediate] addressing, no per-lane address arithmetic
 template <int N>
 struct UnitOff {
     static constexpr int MAXC4 = N - 3;                        // c4 = L-la-1 <= M-2
-    uint16_t a, b, ps, u, v;
-    uint16_t own, w;                                           // per level (same for every la): row of J(i..j), index of 1/P^2
+    uint32_t u, v, w;                                          // scalar tables (w: 1/P^2 of the level's currents)
+    uint16_t a, b, ps;
+    uint16_t own;                                              // per level (same for every la): row of J(i..j)
     uint16_t bm[MAXC4 > 0 ? MAXC4 : 1], c[MAXC4 > 0 ? MAXC4 : 1];
 };
 
@@ -47,16 +49,17 @@ constexpr UnitTable<N> make_unit_table()
         for (int la = 1; la <= L - 1; ++la) {
             UnitOff<N>& o = t.u[UnitTable<N>::index(L, la)];
             const int ra = lv_rowbase<N>(la), rb = lv_rowbase<N>(L - la) + la;
-            o.a = (uint16_t)(ra * D);
-            o.b = (uint16_t)(rb * D);
-            o.ps = (uint16_t)((C::PS0 + la) * D);
-            o.u = (uint16_t)((C::SC_U + ra) * 32);
-            o.v = (uint16_t)((C::SC_V + rb) * 32);
-            o.own = (uint16_t)(lv_rowbase<N>(L) * D);
-            o.w = (uint16_t)((C::SC_W + lv_rowbase<N>(L) - N) * 32);
+            constexpr int EB = (int)sizeof(typename F::E);
+            o.a = (uint16_t)(ra * D * EB);
+            o.b = (uint16_t)(rb * D * EB);
+            o.ps = (uint16_t)((C::PS0 + la) * D * EB);
+            o.u = (uint32_t)((C::SC_U + ra) * 32 * EB);
+            o.v = (uint32_t)((C::SC_V + rb) * 32 * EB);
+            o.own = (uint16_t)(lv_rowbase<N>(L) * D * EB);
+            o.w = (uint32_t)((C::SC_W + lv_rowbase<N>(L) - N) * 32 * EB);
             for (int lb = 1; lb <= L - la - 1; ++lb) {
-                o.bm[lb - 1] = (uint16_t)((lv_rowbase<N>(lb) + la) * D);
-                o.c[lb - 1] = (uint16_t)((lv_rowbase<N>(L - la - lb) + la + lb) * D);
+                o.bm[lb - 1] = (uint16_t)((lv_rowbase<N>(lb) + la) * D * EB);
+                o.c[lb - 1] = (uint16_t)((lv_rowbase<N>(L - la - lb) + la + lb) * D * EB);
             }
         }
     return t;
@@ -72,11 +75,13 @@ __device__ __forceinline__ void unit_body(const typename F::E* __restrict__ ri, 
                                           typename F::A (&acc)[D], typename F::E& hsum)
 {
     typedef typename F::E E;
+    const char* rb_ = reinterpret_cast<const char*>(ri);
+    const char* sb_ = reinterpret_cast<const char*>(si);
     E a[D], b[D], s[D];
-    ld_vec<F, D>(ri + o.a, a);
-    ld_vec<F, D>(ri + o.b, b);
-    ld_vec<F, D>(ri + o.ps, s);                                    // PS2_k, k = i+la-1
-    const E ua = si[o.u], vb = si[o.v];
+    ld_vec<F, D>(reinterpret_cast<const E*>(rb_ + o.a), a);
+    ld_vec<F, D>(reinterpret_cast<const E*>(rb_ + o.b), b);
+    ld_vec<F, D>(reinterpret_cast<const E*>(rb_ + o.ps), s);       // PS2_k, k = i+la-1
+    const E ua = *reinterpret_cast<const E*>(sb_ + o.u), vb = *reinterpret_cast<const E*>(sb_ + o.v);
     const E na0 = F::neg(a[0]);
     const E h = F::neg(F::reduce(dot_neg<F, D>(na0, a, b)));       // A.B
     const E xa = F::reduce(dot_plain<F, D>(x2, a));                // 2 X.A
@@ -106,8 +111,8 @@ __device__ __forceinline__ void unit_body(const typename F::E* __restrict__ ri, 
     for (int q = 0; q < C4; ++q) {
         // (i..k | k+1..l | l+1..j), l = k+q+1: 2 (A.C) J(k+1..l)
         E bm[D], c[D];
-        ld_vec<F, D>(ri + o.bm[q], bm);
-        ld_vec<F, D>(ri + o.c[q], c);
+        ld_vec<F, D>(reinterpret_cast<const E*>(rb_ + o.bm[q]), bm);
+        ld_vec<F, D>(reinterpret_cast<const E*>(rb_ + o.c[q]), c);
         const E cc = F::neg(F::dbl(F::reduce(dot_neg<F, D>(na0, a, c))));
         need(1);
 #pragma unroll
@@ -220,12 +225,12 @@ __global__ void __launch_bounds__(32 * W) bg_unit_kernel(const TileParams<typena
             }
             E v[D];
             if (!top) {
-                const E w = si[widx];
+                const E w = *reinterpret_cast<const E*>(reinterpret_cast<const char*>(si) + widx);
 #pragma unroll
                 for (int mu = 0; mu < D; ++mu) v[mu] = F::mul(F::reduce(acc[mu]), w);
-                st_vec<F, D>(ri + own, v);
+                st_vec<F, D>(reinterpret_cast<E*>(reinterpret_cast<char*>(ri) + own), v);
                 const E c2 = F::reduce(dot_plain<F, D>(x2, v));     // 2 P_{i,j} . J(i..j)
-                const int urow = own / D;
+                const int urow = own / (D * (int)sizeof(E));
                 si[(C::SC_U + urow) * 32] = F::add(c2, hsum);
                 si[(C::SC_V + urow) * 32] = F::sub(c2, hsum);
             } else {
