@@ -38,6 +38,11 @@
  *   errors    return value: BG_OK or a negative bg_status_t; nothing is thrown, nothing
  *             aborts.  Arguments are checked on the host before any launch.  batch == 0 is
  *             a no-op returning BG_OK.
+ *   tuning    two environment variables, read on every call, restrict the kernel selection for A/B
+ *             measurements (they never change results): BG_KERNEL = tile | level | unit | split | reg
+ *             picks a kernel family among the compiled instances of the shape, BG_SWEEP_W = <warps per
+ *             tile> a variant of it, BG_SWEEP_W = 0 the general one-thread-per-point kernel.  Unset
+ *             (the normal case) the default instance of the shape is launched.
  *   1/0       inv(0) := 0 in both fields (what Fermat's a^(p-2) gives); a point where some
  *             proper P_{i,j}^2 vanishes gets status bit0 set (reading R6).
  */
