@@ -19,3 +19,4 @@ struct SweepEntry {
 const SweepEntry* bg_entries_default(int* count);     // bg_inst_default.cu
 const SweepEntry* bg_entries_fp_alt(int* count);      // bg_inst_fp_alt.cu
 const SweepEntry* bg_entries_c128_alt(int* count);    // bg_inst_c128_alt.cu
+const SweepEntry* bg_entries_paper(int* count);       // bg_inst_paper.cu

@@ -247,7 +247,11 @@ VARIANTS = [("fp31", 8, 6, "level", 4), ("fp31", 8, 6, "level", 6), ("fp31", 8, 
             ("c128", 6, 4, "tile", 2), ("fp31", 8, 6, "general", 0), ("c128", 6, 4, "general", 0),
             ("c128", 12, 6, "split", 16), ("c128", 6, 4, "split", 2), ("c128", 6, 4, "split", 4),
             ("c128", 6, 4, "reg", 4), ("fp31", 8, 6, "unit", 4),
-            ("fp31", 10, 8, "unit", 8), ("fp31", 12, 6, "unit", 8)]
+            ("fp31", 10, 8, "unit", 8), ("fp31", 12, 6, "unit", 8),
+            # the shapes of the paper's own benchmarks (bg_inst_paper.cu)
+            ("fp31", 6, 4, "unit", 2), ("fp31", 8, 4, "unit", 4), ("fp31", 9, 4, "unit", 4), ("fp31", 6, 6, "unit", 2),
+            ("fp31", 9, 6, "unit", 4), ("fp31", 6, 8, "unit", 2), ("fp31", 8, 8, "unit", 4), ("fp31", 9, 8, "unit", 4),
+            ("fp31", 6, 10, "unit", 2), ("fp31", 9, 10, "unit", 4)]
 
 
 @pytest.mark.parametrize("field,n,d,kernel,w", VARIANTS, ids=lambda v: str(v))
