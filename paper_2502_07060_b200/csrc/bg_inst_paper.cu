@@ -16,6 +16,13 @@ const SweepEntry* bg_entries_paper(int* count)
         unit_entry<Fp31, 9, 8, 4>(BG_FIELD_FP31),
         unit_entry<Fp31, 6, 10, 2>(BG_FIELD_FP31),
         unit_entry<Fp31, 9, 10, 4>(BG_FIELD_FP31),
+        // the rest of the leg scans n = 4..10 at d = 4 and d = 8 (the configs cover (4,4), (10,8))
+        unit_entry<Fp31, 5, 4, 1>(BG_FIELD_FP31),
+        unit_entry<Fp31, 7, 4, 4>(BG_FIELD_FP31),
+        unit_entry<Fp31, 10, 4, 8>(BG_FIELD_FP31),
+        unit_entry<Fp31, 4, 8, 1>(BG_FIELD_FP31),
+        unit_entry<Fp31, 5, 8, 1>(BG_FIELD_FP31),
+        unit_entry<Fp31, 7, 8, 4>(BG_FIELD_FP31),
     };
     *count = (int)(sizeof(table) / sizeof(table[0]));
     return table;

@@ -152,6 +152,8 @@ extern "C" int bg_selftest_schedules(void)
     if ((rc = check_level_program<10, 8>())) return rc - 60000;
     if ((rc = check_level_program<12, 8>())) return rc - 70000;
     if ((rc = check_level_program<9, 4>())) return rc - 80000;
+    if ((rc = check_level_program<5, 1>())) return rc - 81000;
+    if ((rc = check_level_program<7, 4>())) return rc - 82000;
     if ((rc = check_tile_tables<8, 4>())) return rc - 110000;
     if ((rc = check_tile_tables<8, 8>())) return rc - 120000;
     if ((rc = check_tile_tables<4, 1>())) return rc - 130000;

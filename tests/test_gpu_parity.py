@@ -251,7 +251,8 @@ VARIANTS = [("fp31", 8, 6, "level", 4), ("fp31", 8, 6, "level", 6), ("fp31", 8, 
             # the shapes of the paper's own benchmarks (bg_inst_paper.cu)
             ("fp31", 6, 4, "unit", 2), ("fp31", 8, 4, "unit", 4), ("fp31", 9, 4, "unit", 4), ("fp31", 6, 6, "unit", 2),
             ("fp31", 9, 6, "unit", 4), ("fp31", 6, 8, "unit", 2), ("fp31", 8, 8, "unit", 4), ("fp31", 9, 8, "unit", 4),
-            ("fp31", 6, 10, "unit", 2), ("fp31", 9, 10, "unit", 4)]
+            ("fp31", 6, 10, "unit", 2), ("fp31", 9, 10, "unit", 4), ("fp31", 5, 4, "unit", 1), ("fp31", 7, 4, "unit", 4),
+            ("fp31", 10, 4, "unit", 8), ("fp31", 4, 8, "unit", 1), ("fp31", 5, 8, "unit", 1), ("fp31", 7, 8, "unit", 4)]
 
 
 @pytest.mark.parametrize("field,n,d,kernel,w", VARIANTS, ids=lambda v: str(v))
