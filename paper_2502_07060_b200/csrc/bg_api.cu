@@ -99,7 +99,7 @@ const void* pick(int n, int d, int* s)
 }
 
 // ---- the compile-time (n, d) fast path -------------------------------------------------------------
-// The instances live in four translation units (bg_inst_*.cu): the work lists of a kernel
+// The instances live in several translation units (bg_inst_*.cu): the work lists of a kernel
 // instance sit in constant memory, and one module has 64 KB of it.
 const SweepEntry* find_sweep(int field, int n, int d)
 {
@@ -111,7 +111,8 @@ const SweepEntry* find_sweep(int field, int n, int d)
                                   strcmp(kenv, "split") == 0 ? 2 : strcmp(kenv, "reg") == 0 ? 3 :
                                   strcmp(kenv, "unit") == 0 ? 4 : -1;
     typedef const SweepEntry* (*TableFn)(int*);
-    static const TableFn tables[] = {bg_entries_default, bg_entries_paper, bg_entries_fp_alt, bg_entries_c128_alt};
+    static const TableFn tables[] = {bg_entries_default, bg_entries_paper, bg_entries_grid0, bg_entries_grid1, bg_entries_grid2,
+                                     bg_entries_fp_alt, bg_entries_c128_alt};
     const SweepEntry* first = nullptr;
     for (TableFn fn : tables) {
         int count = 0;

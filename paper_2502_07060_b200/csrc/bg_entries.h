@@ -20,3 +20,6 @@ const SweepEntry* bg_entries_default(int* count);     // bg_inst_default.cu
 const SweepEntry* bg_entries_fp_alt(int* count);      // bg_inst_fp_alt.cu
 const SweepEntry* bg_entries_c128_alt(int* count);    // bg_inst_c128_alt.cu
 const SweepEntry* bg_entries_paper(int* count);       // bg_inst_paper.cu
+const SweepEntry* bg_entries_grid0(int* count);       // bg_inst_grid0.cu
+const SweepEntry* bg_entries_grid1(int* count);       // bg_inst_grid1.cu
+const SweepEntry* bg_entries_grid2(int* count);       // bg_inst_grid2.cu

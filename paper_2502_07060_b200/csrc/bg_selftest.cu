@@ -154,6 +154,7 @@ extern "C" int bg_selftest_schedules(void)
     if ((rc = check_level_program<9, 4>())) return rc - 80000;
     if ((rc = check_level_program<5, 1>())) return rc - 81000;
     if ((rc = check_level_program<7, 4>())) return rc - 82000;
+    if ((rc = check_level_program<4, 1>())) return rc - 83000;
     if ((rc = check_tile_tables<8, 4>())) return rc - 110000;
     if ((rc = check_tile_tables<8, 8>())) return rc - 120000;
     if ((rc = check_tile_tables<4, 1>())) return rc - 130000;

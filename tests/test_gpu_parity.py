@@ -282,3 +282,13 @@ def test_kernel_variants(bgl, oracle_mod, monkeypatch, field, n, d, kernel, w):
         iu = np.triu_indices(n - 1)
         a, b = bgl.to_numpy(cur)[:, iu[0], iu[1]], rcur[:, iu[0], iu[1]]
         assert np.all(np.abs(a - b) <= 1e-8 * (np.abs(b).max(axis=-1, keepdims=True)))
+
+
+# ---- the whole grid n = 4..10 x d = 4..10 over F_p runs a compiled fast-path instance ------------------
+@pytest.mark.parametrize("d", range(4, 11))
+def test_fp_grid_fast_path(bgl, oracle_mod, d):
+    for n in range(4, 11):
+        assert bgl.bg_kernel_info(bgl.FIELD_FP31, n, d)["specialised"] >= 1, (n, d)
+        mom, pol, _ = inputs.make_fp_inputs(n, d, 70, seed=41 + n)          # two full tiles and a ragged one
+        ref = oracle_mod.amplitudes(oracle_mod.FP31, mom, pol, threads=8)
+        assert np.array_equal(_gpu_amplitudes(bgl, mom, pol), ref), (n, d)
