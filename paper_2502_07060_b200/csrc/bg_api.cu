@@ -112,6 +112,7 @@ const SweepEntry* find_sweep(int field, int n, int d)
                                   strcmp(kenv, "unit") == 0 ? 4 : -1;
     typedef const SweepEntry* (*TableFn)(int*);
     static const TableFn tables[] = {bg_entries_default, bg_entries_paper, bg_entries_grid0, bg_entries_grid1, bg_entries_grid2,
+                                     bg_entries_cgrid0, bg_entries_cgrid1,
                                      bg_entries_fp_alt, bg_entries_c128_alt};
     const SweepEntry* first = nullptr;
     for (TableFn fn : tables) {

@@ -23,3 +23,5 @@ const SweepEntry* bg_entries_paper(int* count);       // bg_inst_paper.cu
 const SweepEntry* bg_entries_grid0(int* count);       // bg_inst_grid0.cu
 const SweepEntry* bg_entries_grid1(int* count);       // bg_inst_grid1.cu
 const SweepEntry* bg_entries_grid2(int* count);       // bg_inst_grid2.cu
+const SweepEntry* bg_entries_cgrid0(int* count);      // bg_inst_cgrid0.cu
+const SweepEntry* bg_entries_cgrid1(int* count);      // bg_inst_cgrid1.cu

@@ -164,5 +164,9 @@ extern "C" int bg_selftest_schedules(void)
     if ((rc = check_tile_tables<6, 2>())) return rc - 170000;
     if ((rc = check_tile_tables<16, 8>())) return rc - 180000;
     if ((rc = check_tile_tables<12, 16>())) return rc - 190000;
+    if ((rc = check_tile_tables<4, 2>())) return rc - 200000;
+    if ((rc = check_tile_tables<5, 2>())) return rc - 201000;
+    if ((rc = check_tile_tables<7, 4>())) return rc - 202000;
+    if ((rc = check_tile_tables<9, 8>())) return rc - 203000;
     return rc;
 }

@@ -292,3 +292,15 @@ def test_fp_grid_fast_path(bgl, oracle_mod, d):
         mom, pol, _ = inputs.make_fp_inputs(n, d, 70, seed=41 + n)          # two full tiles and a ragged one
         ref = oracle_mod.amplitudes(oracle_mod.FP31, mom, pol, threads=8)
         assert np.array_equal(_gpu_amplitudes(bgl, mom, pol), ref), (n, d)
+
+
+# ---- complex128: n = 4..10 at d = 4, 6, 8 run a compiled fast-path instance ------------------------------
+@pytest.mark.parametrize("d", [4, 6, 8])
+def test_complex_grid_fast_path(bgl, oracle_mod, d):
+    for n in range(4, 11):
+        assert bgl.bg_kernel_info(bgl.FIELD_C128, n, d)["specialised"] >= 1, (n, d)
+        mom, pol, _ = inputs.make_complex_inputs(n, d, 40, seed=51 + n)     # two full 16-point tiles and a ragged one
+        dbl = oracle_mod.amplitudes(oracle_mod.C128, mom, pol, threads=8)
+        truth = oracle_mod.amplitudes(oracle_mod.C80, mom, pol, threads=8)
+        ok, e_g, _ = _complex_rule(_gpu_amplitudes(bgl, mom, pol), dbl, truth, _kappa(oracle_mod, mom, pol, dbl))
+        assert ok.all() and np.median(e_g) < 1e-12, (n, d, e_g.max())
