@@ -105,5 +105,18 @@ def amplitudes(field: int, momenta: np.ndarray, polarisations: np.ndarray,
     return res[0] if len(res) == 1 else tuple(res)
 
 
+def _sliced(batch: int, threads: int, fn) -> None:
+    """fn(b0, b1) on contiguous slices of [0, batch), one Python thread each"""
+    if threads <= 1 or batch < 2 * threads:
+        fn(0, batch)
+        return
+    bounds = [batch * t // threads for t in range(threads + 1)]
+    ts = [threading.Thread(target=fn, args=(bounds[t], bounds[t + 1])) for t in range(threads)]
+    for t in ts:
+        t.start()
+    for t in ts:
+        t.join()
+
+
 def modulus() -> int:
     return int(_lib().oracle_bg_modulus())

@@ -15,5 +15,7 @@ def pytest_configure(config):
 @pytest.fixture(scope="session")
 def oracle_mod():
     import oracle
+    from oracle import rule
     oracle.build()
+    rule.assert_long_double_is_80_bit()      # the C80 "truth" type of rule R9 must be x87 extended
     return oracle

@@ -279,3 +279,29 @@ def test_multilinearity_in_polarisations(oracle_mod):
     p3[:, 2] = (p3[:, 2] * 3) % P
     a3 = oracle_mod.amplitudes(oracle_mod.FP31, mom, p3.astype(np.uint32)).astype(np.uint64)
     assert np.array_equal(a3, (a0 * 3) % P)
+
+
+def test_truth_type_is_extended_precision(oracle_mod):
+    """rule R9 (oracle/rule.py) uses the long double instantiation as truth: it must carry a 64-bit
+    mantissa and really differ from the double evaluation at rounding level"""
+    from oracle import rule
+    rule.assert_long_double_is_80_bit()
+    mom, pol, _ = inputs.make_complex_inputs(8, 6, 64, seed=2)
+    t = oracle_mod.amplitudes(oracle_mod.C80, mom, pol)
+    dbl = oracle_mod.amplitudes(oracle_mod.C128, mom, pol)
+    assert t.dtype == np.clongdouble
+    rel = (np.abs(dbl.astype(np.clongdouble) - t) / np.abs(t)).astype(np.float64)
+    assert (rel > 0).mean() > 0.9 and rel.max() < 1e-11 and np.median(rel) > 1e-18
+
+
+def test_rule_r9_accepts_the_oracle_and_rejects_a_wrong_result(oracle_mod):
+    from oracle import rule
+    mom, pol, _ = inputs.make_complex_inputs(6, 4, 512, seed=3, helicities=(-1, -1, 1, 1, 1, 1))
+    ref = rule.evaluate(mom, pol, threads=4)
+    ok, st = rule.check(ref["dbl"], ref)
+    assert ok.all() and st["fail"] == 0
+    assert st["pass_by_1e-10"] + st["pass_by_16_e_d"] + st["pass_by_kappa_only"] == 512
+    bad = ref["dbl"].copy()
+    bad[7] *= 1 + 1e-6
+    ok, st = rule.check(bad, ref)
+    assert not ok[7] and st["fail"] >= 1
