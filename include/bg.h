@@ -23,9 +23,14 @@
  * there is no CPU fallback and no other backend.
  *
  * Conventions common to all entry points
- *   scalars   BG_FIELD_FP31: uint32_t residues; values >= p are reduced mod p on load;
+ *   scalars   BG_FIELD_FP31: uint32_t residues mod p = 2^31-1; values >= p are reduced mod p on load;
  *             results are canonical, in [0,p).
  *             BG_FIELD_C128: double[2] = (re, im), interleaved.
+ *             BG_FIELD_FPMONT: uint32_t residues mod a prime 2^30 < p < 2^31 given per call
+ *             (plain residues at the boundary; Montgomery form is internal to the kernels).
+ *   metric    BG_METRIC_MOSTLY_MINUS g = diag(+,-,..,-) unless an entry point takes a
+ *             metric argument; BG_METRIC_ALTERNATING g = diag(+,-,+,-,..) is the switch the paper
+ *             added to match Caravel.
  *   layout    momenta, polarisations: [batch][n][d] scalars, point-major, contravariant
  *             components, all momenta outgoing (sum_l k_l = 0 is the caller's job; the
  *             library evaluates the map above for whatever it is given, reading R4).
@@ -38,11 +43,10 @@
  *   errors    return value: BG_OK or a negative bg_status_t; nothing is thrown, nothing
  *             aborts.  Arguments are checked on the host before any launch.  batch == 0 is
  *             a no-op returning BG_OK.
- *   tuning    two environment variables, read on every call, restrict the kernel selection for A/B
- *             measurements (they never change results): BG_KERNEL = tile | level | unit | split | reg
- *             picks a kernel family among the compiled instances of the shape, BG_SWEEP_W = <warps per
- *             tile> a variant of it, BG_SWEEP_W = 0 the general one-thread-per-point kernel.  Unset
- *             (the normal case) the default instance of the shape is launched.
+ *   tuning    bg_set_kernel_override() restricts the kernel selection for A/B measurements (it never
+ *             changes results); the environment variables BG_KERNEL = unit1 | unit2 | reg | general and
+ *             BG_KERNEL_W = <warps per tile> give its initial value, read ONCE when the library is loaded.
+ *             Without either (the normal case) the default instance of the shape is launched.
  *   1/0       inv(0) := 0 in both fields (what Fermat's a^(p-2) gives); a point where some
  *             proper P_{i,j}^2 vanishes gets status bit0 set (reading R6).
  */
@@ -61,11 +65,13 @@ extern "C" {
 typedef struct CUstream_st* cudaStream_t;
 #endif
 
-typedef enum { BG_FIELD_FP31 = 0, BG_FIELD_C128 = 1 } bg_field_t;
+typedef enum { BG_FIELD_FP31 = 0, BG_FIELD_C128 = 1, BG_FIELD_FPMONT = 2 } bg_field_t;
+typedef enum { BG_METRIC_MOSTLY_MINUS = 0, BG_METRIC_ALTERNATING = 1 } bg_metric_t;
+#define BG_MAX_PRIMES 8
 
 typedef enum {
     BG_OK = 0,
-    BG_ERR_ARG = -1,          /* bad n, d, batch, field, null or misaligned pointer */
+    BG_ERR_ARG = -1,          /* bad n, d, batch, field, metric, prime, null or misaligned pointer */
     BG_ERR_UNSUPPORTED = -2,  /* (field, n, d) needs more shared memory per point than an SM has */
     BG_ERR_CUDA = -3          /* a CUDA runtime call or launch failed */
 } bg_status_t;
@@ -90,6 +96,41 @@ int bg_amplitudes_status(int field, int n, int d, int64_t batch,
 int bg_currents(int field, int n, int d, int64_t batch,
                 const void* momenta, const void* polarisations, void* out,
                 void* currents, uint32_t* status, cudaStream_t stream);
+
+/* ---- the same path, generalised --------------------------------- */
+
+/* What to evaluate.  states = S >= 1 polarisation configurations per momentum point: the partial
+ * momenta, invariants and propagators (rows a1-a3) depend on the momenta only and are formed once
+ * per point, the level sweep runs per configuration -- the workload of the cut equation Eq.(4),
+ * PAPER.md:79-81, whose state sum "runs over all D_s-dimensional particle states".
+ * BG_FIELD_FPMONT: n_primes = 1..BG_MAX_PRIMES primes, each odd and 2^30 < p < 2^31 (primality is the
+ * caller's job: the inverse is a^(p-2)); every array then has a leading [n_primes] axis and prime q
+ * works on slice q (ONE launch, grid.y = n_primes).  Other fields: n_primes = 0. */
+typedef struct {
+    int field;               /* bg_field_t */
+    int metric;              /* bg_metric_t */
+    int n, d;
+    int states;              /* S */
+    int n_primes;
+    uint32_t primes[BG_MAX_PRIMES];
+} bg_problem_t;
+
+/* momenta [P][batch][n][d], polarisations [P][batch][S][n][d], out [P][batch][S], status NULL or
+ * [P][batch] (P = max(1, n_primes)); currents NULL, or [batch][m][m][d] when S == 1 and P == 1.
+ * Device pointers, asynchronous on `stream`. */
+int bg_evaluate(const bg_problem_t* problem, int64_t batch, const void* momenta, const void* polarisations,
+                void* out, void* currents, uint32_t* status, cudaStream_t stream);
+
+/* S state configurations per momentum point, mostly-minus metric (Eq.(4)):
+ * polarisations [batch][S][n][d], out [batch][S]. */
+int bg_amplitudes_states(int field, int n, int d, int64_t batch, int states, const void* momenta,
+                         const void* polarisations, void* out, uint32_t* status, cudaStream_t stream);
+
+/* Several generic 31-bit primes in one launch (Q-reconstruction from the F_p values);
+ * momenta, polarisations [n_primes][batch][n][d] residues mod primes[q], out [n_primes][batch]. */
+int bg_amplitudes_primes(int metric, int n, int d, int64_t batch, int n_primes, const uint32_t* primes,
+                         const void* momenta, const void* polarisations, void* out, uint32_t* status,
+                         cudaStream_t stream);
 
 /* End-to-end variant with HOST buffers (pinned memory recommended): copies the inputs to
  * the device in chunks, runs the kernel and copies the results back, overlapping the three
@@ -119,7 +160,9 @@ typedef struct {
     int64_t mul_v4;          /* 6 d C(n,4) */
     int64_t mul_other;       /* d R + 3(R-1) + d R + d */
     int64_t mul_ref;         /* M_ref = the three above */
-    int64_t mul_factored;    /* field multiplications the kernel's factored form performs */
+    int64_t mul_factored;    /* field multiplications the kernels' factored form executes (bg_common.cuh):
+                                6d per 3-split, 2d per 4-split, per current d (boundary term) + d (propagator)
+                                + d (2P.J) + 1, per single gluon d, d R invariants, 3(R-1) + ~45 batch inverse */
     int64_t bytes_in;        /* 2 n d w */
     int64_t bytes_out;       /* w */
 } bg_opcount_t;
@@ -127,8 +170,9 @@ int bg_op_count(int field, int n, int d, bg_opcount_t* out);
 
 /* Launch configuration the library would use for (field, n, d). */
 typedef struct {
-    int specialised;         /* 0: runtime-n kernel; (n, d) compiled in: 1 table-driven tile kernel,
-                                2 level-unrolled kernel (the one a call would launch) */
+    int specialised;         /* 0: bg_general_kernel (run-time n, one thread per point); (n, d) compiled in:
+                                1 bg_unit_kernel with one lane per point, 2 bg_unit_kernel with two lanes per
+                                point, 3 bg_reg_kernel (currents in registers) -- the one a call would launch */
     int threads_per_block;
     int points_per_block;
     int smem_bytes_per_block;
@@ -136,7 +180,14 @@ typedef struct {
     int blocks_per_sm;       /* limited by shared memory */
     int regs_per_thread;
 } bg_kernel_info_t;
-int bg_kernel_info(int field, int n, int d, bg_kernel_info_t* out);
+int bg_kernel_info(int field, int n, int d, bg_kernel_info_t* out);             /* mostly-minus metric, S = 1 */
+int bg_kernel_info_problem(const bg_problem_t* problem, bg_kernel_info_t* out);
+
+/* Restrict the kernel selection of all later calls (process-wide; for A/B measurements, not meant to
+ * be changed while other threads are inside the library).  kind: -1 default, 1 / 2 / 3 as in
+ * bg_kernel_info_t.specialised, 0 the general kernel; warps: warps per tile, 0 = the first instance
+ * of that kind.  A shape with no matching instance falls back to its default.  Returns BG_OK. */
+int bg_set_kernel_override(int kind, int warps);
 
 /* Host-side self-check of the compile-time work schedules of the tiled kernels (every splitting
  * of Eq.(6), executed exactly once; parts of a shared current gathered exactly once;

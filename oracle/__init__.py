@@ -44,6 +44,8 @@ def _lib():
         lib.oracle_bg_amplitudes.argtypes = [ci, ci, ci, i64, vp, vp, vp, vp]
         lib.oracle_bg_amplitudes.restype = ci
         lib.oracle_bg_modulus.restype = ctypes.c_uint32
+        lib.oracle_bg_evaluate.argtypes = [ci, ci, ctypes.c_uint32, ci, ci, i64, ci, vp, vp, vp, vp, vp]
+        lib.oracle_bg_evaluate.restype = ci
         _LIB = lib
     return _LIB
 
@@ -58,51 +60,61 @@ def _dtypes(field: int):
     raise ValueError("field must be FP31, C128 or C80")
 
 
-def amplitudes(field: int, momenta: np.ndarray, polarisations: np.ndarray,
-               want_currents: bool = False, want_status: bool = False, threads: int = 1):
-    """momenta, polarisations: [batch, n, d].  Returns out [batch] (and, on request,
-    currents [batch, m, m, d] and status [batch]).  threads > 1 splits the batch into
+MOSTLY_MINUS, ALTERNATING = 0, 1
+
+
+def evaluate(field: int, momenta: np.ndarray, polarisations: np.ndarray, metric: int = MOSTLY_MINUS,
+             prime: int = 0, want_currents: bool = False, want_status: bool = False, threads: int = 1):
+    """The literal recursion for momenta [batch, n, d] and polarisations [batch, n, d] or, with S
+    state configurations per momentum point (Eq.(4)), [batch, S, n, d].
+    metric: MOSTLY_MINUS or ALTERNATING; prime (FP31 only): 0 for
+    2^31-1, else any prime below 2^31.  Returns out [batch] / [batch, S] (and, on request,
+    currents [batch, (S,) m, m, d] and status [batch]).  threads > 1 splits the batch into
     contiguous slices, one Python thread each (ctypes releases the GIL)."""
     in_dt, out_dt = _dtypes(field)
     mom = np.ascontiguousarray(momenta, dtype=in_dt)
     pol = np.ascontiguousarray(polarisations, dtype=in_dt)
-    if mom.ndim != 3 or mom.shape != pol.shape:
-        raise ValueError("momenta and polarisations must both be [batch, n, d]")
+    has_states = pol.ndim == 4
+    if mom.ndim != 3 or pol.ndim not in (3, 4) or pol.shape[0] != mom.shape[0] or pol.shape[-2:] != mom.shape[1:]:
+        raise ValueError("momenta must be [batch, n, d], polarisations [batch, n, d] or [batch, S, n, d]")
     batch, n, d = mom.shape
+    S = pol.shape[1] if has_states else 1
     m = n - 1
-    out = np.zeros(batch, dtype=out_dt)
-    cur = np.zeros((batch, m, m, d), dtype=out_dt) if want_currents else None
+    out = np.zeros((batch, S), dtype=out_dt)
+    cur = np.zeros((batch, S, m, m, d), dtype=out_dt) if want_currents else None
     status = np.zeros(batch, dtype=np.uint32)
     lib = _lib()
-    rc = [0] * max(1, threads)
+    bad = []
 
-    def run(t, b0, b1):
-        if b1 <= b0:
-            return
-        rc[t] = lib.oracle_bg_currents(
-            field, n, d, b1 - b0, mom[b0:b1].ctypes.data, pol[b0:b1].ctypes.data,
-            out[b0:b1].ctypes.data, None if cur is None else cur[b0:b1].ctypes.data,
-            status[b0:b1].ctypes.data)
+    def run(b0, b1):
+        if b1 > b0 and lib.oracle_bg_evaluate(
+                field, metric, prime, n, d, b1 - b0, S, mom[b0:b1].ctypes.data, pol[b0:b1].ctypes.data,
+                out[b0:b1].ctypes.data, None if cur is None else cur[b0:b1].ctypes.data,
+                status[b0:b1].ctypes.data):
+            bad.append(b0)
 
-    if threads <= 1 or batch < 2 * threads:
-        rc[0] = lib.oracle_bg_currents(
-            field, n, d, batch, mom.ctypes.data, pol.ctypes.data, out.ctypes.data,
-            None if cur is None else cur.ctypes.data, status.ctypes.data)
+    if batch == 0:
+        if lib.oracle_bg_evaluate(field, metric, prime, n, d, 0, S, None, None, None, None, None):
+            bad.append(0)
     else:
-        bounds = [batch * t // threads for t in range(threads + 1)]
-        ts = [threading.Thread(target=run, args=(t, bounds[t], bounds[t + 1])) for t in range(threads)]
-        for t in ts:
-            t.start()
-        for t in ts:
-            t.join()
-    if any(r != 0 for r in rc):
-        raise ValueError("oracle rejected the arguments (need 4<=n<=16, 4<=d<=16)")
+        _sliced(batch, threads, run)
+    if bad:
+        raise ValueError("oracle rejected the arguments (need 4<=n<=16, 4<=d<=16, metric 0|1, prime < 2^31)")
+    if not has_states:
+        out = out[:, 0]
+        cur = None if cur is None else cur[:, 0]
     res = [out]
     if want_currents:
         res.append(cur)
     if want_status:
         res.append(status)
     return res[0] if len(res) == 1 else tuple(res)
+
+
+def amplitudes(field: int, momenta: np.ndarray, polarisations: np.ndarray,
+               want_currents: bool = False, want_status: bool = False, threads: int = 1):
+    """evaluate() with the mostly-minus metric, p = 2^31-1 and one state configuration"""
+    return evaluate(field, momenta, polarisations, MOSTLY_MINUS, 0, want_currents, want_status, threads)
 
 
 def _sliced(batch: int, threads: int, fn) -> None:

@@ -12,8 +12,12 @@
  * with every lower current J(i..j) = bracket / P_{i,j}^2; see bg_recursion.inc,
  * which follows Eq.(6)/(7) term by term in the paper's order and notation.
  *
+ * Metric: g = diag(+,-,...,-) or, on request, Caravel's alternating
+ * diag(+,-,+,-,...) ("a modification of the metric in our code").
+ *
  * Number types:
- *   field 0  F_p, p = 2^31-1: uint32 residues, every operation is uint64 `% p`,
+ *   field 0  F_p, p = 2^31-1 or any other prime below 2^31 given by the caller (the paper never
+ *            names its prime): uint32 residues, every operation is uint64 `% p`,
  *            one Fermat inverse a^(p-2) by square-and-multiply PER propagator
  *            (no batching trick here on purpose).  Inputs >= p are reduced on load.
  *   field 1  complex128: C99 `double _Complex`, compiled with -ffp-contract=off,
@@ -36,21 +40,27 @@
 
 #define BG_P31 2147483647ULL
 
+/* the prime and the metric of the evaluation in progress (set per call, per thread) */
+static _Thread_local uint64_t bg_p = BG_P31;
+static _Thread_local int bg_alternating = 0;
+/* g_{mu mu} = -1 ?   mostly minus: every mu >= 1; alternating: odd mu */
+static int metric_minus(int mu) { return bg_alternating ? (mu & 1) : (mu >= 1); }
+
 /* ---------------------------------------------------------------- F_p ---- */
-static uint32_t fp_add(uint32_t a, uint32_t b) { return (uint32_t)(((uint64_t)a + b) % BG_P31); }
-static uint32_t fp_sub(uint32_t a, uint32_t b) { return (uint32_t)(((uint64_t)a + BG_P31 - b) % BG_P31); }
-static uint32_t fp_mul(uint32_t a, uint32_t b) { return (uint32_t)(((uint64_t)a * b) % BG_P31); }
+static uint32_t fp_add(uint32_t a, uint32_t b) { return (uint32_t)(((uint64_t)a + b) % bg_p); }
+static uint32_t fp_sub(uint32_t a, uint32_t b) { return (uint32_t)(((uint64_t)a + bg_p - b) % bg_p); }
+static uint32_t fp_mul(uint32_t a, uint32_t b) { return (uint32_t)(((uint64_t)a * b) % bg_p); }
 static uint32_t fp_inv(uint32_t a)
 {   /* Fermat: a^(p-2); gives 0 for a = 0 */
-    uint64_t r = 1, base = a, e = BG_P31 - 2;
+    uint64_t r = 1, base = a, e = bg_p - 2;
     while (e) {
-        if (e & 1) r = (r * base) % BG_P31;
-        base = (base * base) % BG_P31;
+        if (e & 1) r = (r * base) % bg_p;
+        base = (base * base) % bg_p;
         e >>= 1;
     }
     return (uint32_t)r;
 }
-static uint32_t fp_load(const void* p, long idx) { return (uint32_t)(((const uint32_t*)p)[idx] % BG_P31); }
+static uint32_t fp_load(const void* p, long idx) { return (uint32_t)(((const uint32_t*)p)[idx] % bg_p); }
 
 #define SCALAR uint32_t
 #define S_ZERO 0u
@@ -135,35 +145,56 @@ static int check_args(int field, int n, int d, int64_t batch)
 }
 
 /* All pointers are HOST pointers; caller owns every buffer.
- *   momenta, polarisations: [batch][n][d] scalars (uint32 | double[2] | double[2])
- *   out:      [batch] scalars (uint32 | double[2] | long double[2])
- *   currents: NULL or [batch][m][m][d] scalars of the output type, m = n-1
+ *   metric:   0 mostly minus, 1 alternating
+ *   prime:    field 0 only: 0 = 2^31-1, else a prime 2 < prime < 2^31 (primality is the caller's job)
+ *   states:   S >= 1 polarisation configurations per momentum point (the state sum of Eq.(4),
+ *             PAPER.md:79-81): the literal recursion is simply run S times, nothing is shared
+ *   momenta:  [batch][n][d] scalars (uint32 | double[2] | double[2]);
+ *   polarisations: [batch][S][n][d]
+ *   out:      [batch][S] scalars (uint32 | double[2] | long double[2])
+ *   currents: NULL or [batch][S][m][m][d] scalars of the output type, m = n-1
  *             (entry (i-1,j-1) = J(i..j) for i<=j; the top one without propagator)
  *   status:   NULL or [batch] uint32, bit0 = some proper P_{i,j}^2 == 0
  * Returns 0, or -1 on bad arguments.  Single-threaded: callers that want more
- * cores call it on disjoint batch slices from several threads (it keeps no
- * global state). */
-int oracle_bg_currents(int field, int n, int d, int64_t batch, const void* momenta,
-                       const void* polarisations, void* out, void* currents, uint32_t* status)
+ * cores call it on disjoint batch slices from several threads. */
+int oracle_bg_evaluate(int field, int metric, uint32_t prime, int n, int d, int64_t batch, int states,
+                       const void* momenta, const void* polarisations, void* out, void* currents,
+                       uint32_t* status)
 {
     if (check_args(field, n, d, batch) || (batch > 0 && (!momenta || !polarisations || !out))) return -1;
+    if ((metric != 0 && metric != 1) || states < 1 || (field == ORACLE_FP31 && prime == 1)) return -1;
+    if (field == ORACLE_FP31 && prime >= 0x80000000u) return -1;
+    bg_p = (field == ORACLE_FP31 && prime) ? prime : BG_P31;
+    bg_alternating = metric;
     const int m = n - 1;
     const long nd = (long)n * d, cur = (long)m * m * d;
     for (int64_t b = 0; b < batch; ++b) {
         unsigned st = 0;
-        if (field == ORACLE_FP31) {
-            uint32_t* J = currents ? (uint32_t*)currents + b * cur : NULL;
-            ((uint32_t*)out)[b] = fp31_point(n, d, momenta, polarisations, b * nd, J, &st);
-        } else if (field == ORACLE_C128) {
-            c128* J = currents ? (c128*)currents + b * cur : NULL;
-            ((c128*)out)[b] = c128_point(n, d, momenta, polarisations, b * nd, J, &st);
-        } else {
-            c80* J = currents ? (c80*)currents + b * cur : NULL;
-            ((c80*)out)[b] = c80_point(n, d, momenta, polarisations, b * nd, J, &st);
+        for (int s = 0; s < states; ++s) {
+            const int64_t o = b * states + s;
+            if (field == ORACLE_FP31) {
+                uint32_t* J = currents ? (uint32_t*)currents + o * cur : NULL;
+                ((uint32_t*)out)[o] = fp31_point(n, d, momenta, polarisations, b * nd, o * nd, J, &st);
+            } else if (field == ORACLE_C128) {
+                c128* J = currents ? (c128*)currents + o * cur : NULL;
+                ((c128*)out)[o] = c128_point(n, d, momenta, polarisations, b * nd, o * nd, J, &st);
+            } else {
+                c80* J = currents ? (c80*)currents + o * cur : NULL;
+                ((c80*)out)[o] = c80_point(n, d, momenta, polarisations, b * nd, o * nd, J, &st);
+            }
         }
         if (status) status[b] = st;
     }
+    bg_p = BG_P31;
+    bg_alternating = 0;
     return 0;
+}
+
+/* mostly-minus metric, p = 2^31-1, one state configuration */
+int oracle_bg_currents(int field, int n, int d, int64_t batch, const void* momenta,
+                       const void* polarisations, void* out, void* currents, uint32_t* status)
+{
+    return oracle_bg_evaluate(field, 0, 0, n, d, batch, 1, momenta, polarisations, out, currents, status);
 }
 
 int oracle_bg_amplitudes(int field, int n, int d, int64_t batch, const void* momenta,

@@ -16,15 +16,19 @@ import numpy as np
 
 from . import build as _build
 
-FIELD_FP31, FIELD_C128 = 0, 1
+FIELD_FP31, FIELD_C128, FIELD_FPMONT = 0, 1, 2
+METRIC_MOSTLY_MINUS, METRIC_ALTERNATING = 0, 1
+MAX_PRIMES = 8
+KERNEL_KINDS = {"default": -1, "general": 0, "unit1": 1, "unit2": 2, "reg": 3}
 BG_OK, BG_ERR_ARG, BG_ERR_UNSUPPORTED, BG_ERR_CUDA = 0, -1, -2, -3
 PEAK_KINDS = {"imad_wide": 0, "imad": 1, "alu": 2, "mix": 3, "modmul": 4, "dfma": 5,
               "lds32": 6, "lds64": 7, "lds128": 8, "mix2": 9, "mix3": 10, "imad_wide_rz": 11}
 P31 = (1 << 31) - 1
 
-EXPORTS = ["bg_amplitudes", "bg_amplitudes_status", "bg_currents", "bg_amplitudes_host",
-           "bg_host_workspace_bytes", "bg_modulus", "bg_status_string", "bg_version",
-           "bg_op_count", "bg_kernel_info", "bg_peak_probe", "bg_selftest_schedules"]
+EXPORTS = ["bg_amplitudes", "bg_amplitudes_status", "bg_currents", "bg_evaluate", "bg_amplitudes_states",
+           "bg_amplitudes_primes", "bg_amplitudes_host", "bg_host_workspace_bytes", "bg_modulus",
+           "bg_status_string", "bg_version", "bg_op_count", "bg_kernel_info", "bg_kernel_info_problem",
+           "bg_set_kernel_override", "bg_peak_probe", "bg_selftest_schedules"]
 
 
 class BgError(RuntimeError):
@@ -35,6 +39,19 @@ class OpCount(ctypes.Structure):
     _fields_ = [(k, ctypes.c_int64) for k in
                 ("currents", "propagators", "splits3", "splits4", "mul_v3", "mul_v4", "mul_other",
                  "mul_ref", "mul_factored", "bytes_in", "bytes_out")]
+
+
+class Problem(ctypes.Structure):
+    """bg_problem_t"""
+    _fields_ = [("field", ctypes.c_int), ("metric", ctypes.c_int), ("n", ctypes.c_int), ("d", ctypes.c_int),
+                ("states", ctypes.c_int), ("n_primes", ctypes.c_int), ("primes", ctypes.c_uint32 * MAX_PRIMES)]
+
+
+def problem(field, n, d, metric=METRIC_MOSTLY_MINUS, states=1, primes=()) -> Problem:
+    pb = Problem(field, metric, n, d, states, len(primes))
+    for i, p in enumerate(primes):
+        pb.primes[i] = p
+    return pb
 
 
 class KernelInfo(ctypes.Structure):
@@ -65,6 +82,11 @@ def load(rebuild_if_stale: bool = False):
     lib.bg_amplitudes.argtypes = [ci, ci, ci, i64, vp, vp, vp, vp]
     lib.bg_amplitudes_status.argtypes = [ci, ci, ci, i64, vp, vp, vp, vp, vp]
     lib.bg_currents.argtypes = [ci, ci, ci, i64, vp, vp, vp, vp, vp, vp]
+    lib.bg_evaluate.argtypes = [ctypes.POINTER(Problem), i64, vp, vp, vp, vp, vp, vp]
+    lib.bg_amplitudes_states.argtypes = [ci, ci, ci, i64, ci, vp, vp, vp, vp, vp]
+    lib.bg_amplitudes_primes.argtypes = [ci, ci, ci, i64, ci, ctypes.POINTER(ctypes.c_uint32), vp, vp, vp, vp, vp]
+    lib.bg_kernel_info_problem.argtypes = [ctypes.POINTER(Problem), ctypes.POINTER(KernelInfo)]
+    lib.bg_set_kernel_override.argtypes = [ci, ci]
     lib.bg_amplitudes_host.argtypes = [ci, ci, ci, i64, vp, vp, vp, vp, vp, sz]
     lib.bg_host_workspace_bytes.argtypes = [ci, ci, ci, i64]
     lib.bg_host_workspace_bytes.restype = sz
@@ -75,8 +97,9 @@ def load(rebuild_if_stale: bool = False):
     lib.bg_op_count.argtypes = [ci, ci, ci, ctypes.POINTER(OpCount)]
     lib.bg_kernel_info.argtypes = [ci, ci, ci, ctypes.POINTER(KernelInfo)]
     lib.bg_peak_probe.argtypes = [ci, ci, ci, ci, vp, ctypes.POINTER(i64), vp]
-    for name in ("bg_amplitudes", "bg_amplitudes_status", "bg_currents", "bg_amplitudes_host",
-                 "bg_op_count", "bg_kernel_info", "bg_peak_probe"):
+    for name in ("bg_amplitudes", "bg_amplitudes_status", "bg_currents", "bg_amplitudes_host", "bg_evaluate",
+                 "bg_amplitudes_states", "bg_amplitudes_primes", "bg_kernel_info_problem",
+                 "bg_set_kernel_override", "bg_op_count", "bg_kernel_info", "bg_peak_probe"):
         getattr(lib, name).restype = ci
     _LIB = lib
     return lib
@@ -102,6 +125,36 @@ def bg_currents(field, n, d, batch, momenta_ptr, polarisations_ptr, out_ptr, cur
                 stream_ptr=0):
     return load().bg_currents(field, n, d, batch, momenta_ptr, polarisations_ptr, out_ptr,
                               currents_ptr, status_ptr, stream_ptr)
+
+
+def bg_evaluate(pb: Problem, batch, momenta_ptr, polarisations_ptr, out_ptr, currents_ptr=None, status_ptr=None,
+                stream_ptr=0):
+    return load().bg_evaluate(ctypes.byref(pb), batch, momenta_ptr, polarisations_ptr, out_ptr, currents_ptr,
+                              status_ptr, stream_ptr)
+
+
+def bg_amplitudes_states(field, n, d, batch, states, momenta_ptr, polarisations_ptr, out_ptr, status_ptr=None,
+                         stream_ptr=0):
+    return load().bg_amplitudes_states(field, n, d, batch, states, momenta_ptr, polarisations_ptr, out_ptr,
+                                       status_ptr, stream_ptr)
+
+
+def bg_amplitudes_primes(metric, n, d, batch, primes, momenta_ptr, polarisations_ptr, out_ptr, status_ptr=None,
+                         stream_ptr=0):
+    arr = (ctypes.c_uint32 * len(primes))(*primes)
+    return load().bg_amplitudes_primes(metric, n, d, batch, len(primes), arr, momenta_ptr, polarisations_ptr,
+                                       out_ptr, status_ptr, stream_ptr)
+
+
+def bg_set_kernel_override(kind=-1, warps=0):
+    """kind: -1 / "default", or "general", "unit1", "unit2", "reg" (bg.h)"""
+    return load().bg_set_kernel_override(KERNEL_KINDS[kind] if isinstance(kind, str) else kind, warps)
+
+
+def bg_kernel_info_problem(pb: Problem) -> dict:
+    ki = KernelInfo()
+    _check(load().bg_kernel_info_problem(ctypes.byref(pb), ctypes.byref(ki)))
+    return {k: int(getattr(ki, k)) for k, _ in KernelInfo._fields_}
 
 
 def bg_amplitudes_host(field, n, d, batch, host_mom_ptr, host_pol_ptr, host_out_ptr, host_status_ptr,
@@ -205,6 +258,31 @@ def amplitudes(momenta, polarisations, out=None, status=None, stream=None):
         else:
             _check(bg_amplitudes_status(field, n, d, batch, momenta.data_ptr(), polarisations.data_ptr(),
                                         out.data_ptr(), status.data_ptr(), s))
+    return out
+
+
+def evaluate(momenta, polarisations, metric=METRIC_MOSTLY_MINUS, primes=(), status=None, stream=None):
+    """The generalised path (bg_evaluate).  momenta [B,n,d] (with primes: [P,B,n,d]); polarisations the same
+    shape, or with a state axis [B,S,n,d] ([P,B,S,n,d]).  Returns out [B] / [B,S] (leading [P] with primes)."""
+    torch = _torch()
+    lead = 1 if primes else 0
+    if momenta.dim() != 3 + lead or polarisations.dim() not in (3 + lead, 4 + lead):
+        raise BgError("bad tensor ranks for evaluate()")
+    if not (momenta.is_cuda and polarisations.is_cuda and momenta.is_contiguous() and polarisations.is_contiguous()):
+        raise BgError("inputs must be contiguous CUDA tensors")
+    batch, n, d = (int(x) for x in momenta.shape[lead:])
+    has_states = polarisations.dim() == 4 + lead
+    states = int(polarisations.shape[lead + 1]) if has_states else 1
+    field = FIELD_FPMONT if primes else field_of(momenta)
+    if primes and (field_of(momenta) != FIELD_FP31 or momenta.shape[0] != len(primes)):
+        raise BgError("with primes the inputs are uint32/int32 residues with a leading [len(primes)] axis")
+    shape = ([len(primes)] if primes else []) + [batch] + ([states] if has_states else [])
+    out = torch.empty(shape, dtype=momenta.dtype, device=momenta.device)
+    pb = problem(field, n, d, metric, states, tuple(primes))
+    s = (stream or torch.cuda.current_stream(momenta.device)).cuda_stream
+    with torch.cuda.device(momenta.device):
+        _check(bg_evaluate(pb, batch, momenta.data_ptr(), polarisations.data_ptr(), out.data_ptr(), None,
+                           None if status is None else status.data_ptr(), s))
     return out
 
 

@@ -2,225 +2,266 @@
 // The C ABI is declared and documented in include/bg.h.
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdlib.h>
 #include <string.h>
 
+#include <atomic>
+#include <mutex>
+
 #include "../../include/bg.h"
-#include "bg_recursion.cuh"
-#include "bg_tile.cuh"      // TileParams
+#include "bg_common.cuh"
 #include "bg_entries.h"
-#include <stdlib.h>
+#include "bg_general.cuh"     // GeneralLayout (host side of the record layout)
 
 namespace {
 
+using bg::BgParams;
 using bg::C128;
 using bg::Fp31;
-using bg::KernelParams;
+using bg::FpMont;
 
 constexpr int kMaxSmemPerBlock = 232448;   // 227 KB opt-in limit per CTA on sm_100
 constexpr int kSmemPerSm = 233472;         // 228 KB per SM
 constexpr int kSmemReservedPerBlock = 1024;
+constexpr int kMaxDevices = 64;
 
-struct LaunchPlan {
-    const void* func;
-    int specialised;
-    int threads;
-    int stride;            // record stride in elements
-    int elem_bytes;
-    int smem_bytes;
+// ---- kernel selection ------------------------------------------------------------------------------
+// What a call launches, resolved ONCE per (field, metric, n, d, needs-states) and cached; the
+// steady-state call path does no table scan, no getenv and no cudaFuncSetAttribute.
+struct Launch {
+    const void* func = nullptr;
+    int kind = BG_KIND_GENERAL;        // BgKernelKind
+    int threads = 0;
+    int points_per_block = 0;
+    int smem = 0;
+    int stride = 0;                    // general kernel: record stride in elements
+    std::atomic<uint64_t> attr_done{0};   // bit i: cudaFuncSetAttribute done on device i
 };
 
-template <class F, int N, int D>
-const void* kernel_ptr()
-{
-    return reinterpret_cast<const void*>(&bg::bg_recursion_kernel<F, N, D>);
-}
+std::atomic<int> g_override_kind{-1};   // bg_kernel_info_t.specialised numbering; -1 = default
+std::atomic<int> g_override_w{0};
 
-template <class F, int D>
-const void* pick_d(int n, int* specialised);
-
-// the (n, d) pairs of BASELINE.json:configs get fully compile-time instances
-template <>
-const void* pick_d<Fp31, 4>(int n, int* s)
-{
-    if (n == 4) { *s = 1; return kernel_ptr<Fp31, 4, 4>(); }
-    *s = 0; return kernel_ptr<Fp31, 0, 4>();
-}
-template <>
-const void* pick_d<Fp31, 6>(int n, int* s)
-{
-    if (n == 8) { *s = 1; return kernel_ptr<Fp31, 8, 6>(); }
-    if (n == 12) { *s = 1; return kernel_ptr<Fp31, 12, 6>(); }
-    *s = 0; return kernel_ptr<Fp31, 0, 6>();
-}
-template <>
-const void* pick_d<Fp31, 8>(int n, int* s)
-{
-    if (n == 10) { *s = 1; return kernel_ptr<Fp31, 10, 8>(); }
-    *s = 0; return kernel_ptr<Fp31, 0, 8>();
-}
-template <>
-const void* pick_d<C128, 4>(int n, int* s)
-{
-    if (n == 6) { *s = 1; return kernel_ptr<C128, 6, 4>(); }
-    *s = 0; return kernel_ptr<C128, 0, 4>();
-}
-template <>
-const void* pick_d<C128, 6>(int n, int* s)
-{
-    if (n == 12) { *s = 1; return kernel_ptr<C128, 12, 6>(); }
-    *s = 0; return kernel_ptr<C128, 0, 6>();
-}
-template <class F, int D>
-const void* pick_d(int, int* s)
-{
-    *s = 0;
-    return kernel_ptr<F, 0, D>();
-}
-
-template <class F>
-const void* pick(int n, int d, int* s)
-{
-    switch (d) {
-        case 4: return pick_d<F, 4>(n, s);
-        case 5: return pick_d<F, 5>(n, s);
-        case 6: return pick_d<F, 6>(n, s);
-        case 7: return pick_d<F, 7>(n, s);
-        case 8: return pick_d<F, 8>(n, s);
-        case 9: return pick_d<F, 9>(n, s);
-        case 10: return pick_d<F, 10>(n, s);
-        case 11: return pick_d<F, 11>(n, s);
-        case 12: return pick_d<F, 12>(n, s);
-        case 13: return pick_d<F, 13>(n, s);
-        case 14: return pick_d<F, 14>(n, s);
-        case 15: return pick_d<F, 15>(n, s);
-        case 16: return pick_d<F, 16>(n, s);
-    }
-    return nullptr;
-}
-
-// ---- the compile-time (n, d) fast path -------------------------------------------------------------
-// The instances live in several translation units (bg_inst_*.cu): the work lists of a kernel
-// instance sit in constant memory, and one module has 64 KB of it.
-const SweepEntry* find_sweep(int field, int n, int d)
-{
-    const char* env = getenv("BG_SWEEP_W");
-    const int want = env ? atoi(env) : 0;
-    if (env && want == 0) return nullptr;            // BG_SWEEP_W=0: force the runtime-n kernel
-    const char* kenv = getenv("BG_KERNEL");          // restrict the kernel family (A/B runs)
-    const int kind = !kenv ? -1 : strcmp(kenv, "tile") == 0 ? 0 : strcmp(kenv, "level") == 0 ? 1 :
-                                  strcmp(kenv, "split") == 0 ? 2 : strcmp(kenv, "reg") == 0 ? 3 :
-                                  strcmp(kenv, "unit") == 0 ? 4 : -1;
-    typedef const SweepEntry* (*TableFn)(int*);
-    static const TableFn tables[] = {bg_entries_default, bg_entries_paper, bg_entries_grid0, bg_entries_grid1, bg_entries_grid2,
-                                     bg_entries_cgrid0, bg_entries_cgrid1,
-                                     bg_entries_fp_alt, bg_entries_c128_alt};
-    const SweepEntry* first = nullptr;
-    for (TableFn fn : tables) {
-        int count = 0;
-        const SweepEntry* t = fn(&count);
-        for (int i = 0; i < count; ++i) {
-            if (t[i].field != field || t[i].n != n || t[i].d != d) continue;
-            if (kind >= 0 && t[i].kind != kind) continue;
-            if (t[i].smem > (size_t)kMaxSmemPerBlock) continue;
-            if (!first) first = &t[i];
-            if (t[i].w == want) return &t[i];
+struct EnvInit {
+    EnvInit()
+    {   // initial value of the override, read once at load time (bg.h "tuning")
+        const char* k = getenv("BG_KERNEL");
+        const char* w = getenv("BG_KERNEL_W");
+        if (k) {
+            g_override_kind = strcmp(k, "general") == 0 ? 0 : strcmp(k, "unit1") == 0 ? 1 :
+                              strcmp(k, "unit2") == 0 ? 2 : strcmp(k, "reg") == 0 ? 3 : -1;
         }
+        if (w) g_override_w = atoi(w);
     }
-    return first;
-}
+} g_env_init;
 
+int elem_bytes(int field) { return field == BG_FIELD_C128 ? 16 : 4; }
 int vec_width(int field, int d)
 {
     if (field == BG_FIELD_C128) return 1;
     return (d % 4 == 0) ? 4 : (d % 2 == 0) ? 2 : 1;
 }
 
-int check_shape(int field, int n, int d)
+const KernelEntry* find_entry(int field, int metric, int n, int d, bool multi_state, int want_kind, int want_w)
 {
-    if (field != BG_FIELD_FP31 && field != BG_FIELD_C128) return BG_ERR_ARG;
+    typedef const KernelEntry* (*TableFn)(int*);
+#define BG_TABLE_PTR(name) bg_entries_##name,
+    static const TableFn tables[] = {BG_ENTRY_TABLES(BG_TABLE_PTR)};
+#undef BG_TABLE_PTR
+    const KernelEntry* first = nullptr;
+    for (TableFn fn : tables) {
+        int count = 0;
+        const KernelEntry* t = fn(&count);
+        for (int i = 0; i < count; ++i) {
+            const KernelEntry& e = t[i];
+            if (e.field != field || e.metric != metric || e.n != n || e.d != d) continue;
+            if (e.smem > (size_t)kMaxSmemPerBlock) continue;
+            if (multi_state && e.kind == BG_KIND_REG) continue;         // bg_reg_kernel: one configuration only
+            if (want_kind >= 0 && e.kind != want_kind) continue;
+            if (!first) first = &e;
+            if (want_w == 0 || e.w == want_w) return &e;
+        }
+    }
+    return first;
+}
+
+const void* general_ptr(int field, int metric, int d)
+{
+    switch (field) {
+        case BG_FIELD_FP31: return bg_general_kernel_ptr_fp31(metric, d);
+        case BG_FIELD_C128: return bg_general_kernel_ptr_c128(metric, d);
+        case BG_FIELD_FPMONT: return bg_general_kernel_ptr_mont(metric, d);
+    }
+    return nullptr;
+}
+
+int fill_general(int field, int metric, int n, int d, Launch* L)
+{
+    const bg::GeneralLayout lay = bg::make_general_layout(n, d, vec_width(field, d));
+    const int per_point = lay.stride * elem_bytes(field);
+    int t = kMaxSmemPerBlock / per_point;
+    if (t < 1) return BG_ERR_UNSUPPORTED;
+    if (t > 32) t = 32;
+    L->func = general_ptr(field, metric, d);
+    if (!L->func) return BG_ERR_UNSUPPORTED;
+    L->kind = BG_KIND_GENERAL;
+    L->threads = t;
+    L->points_per_block = t;
+    L->smem = t * per_point;
+    L->stride = lay.stride;
+    return BG_OK;
+}
+
+void fill_entry(const KernelEntry& e, Launch* L)
+{
+    L->func = e.func;
+    L->kind = e.kind;
+    L->threads = 32 * e.w;
+    L->points_per_block = e.tp;
+    L->smem = (int)e.smem;
+    L->stride = 0;
+}
+
+int check_shape(int field, int metric, int n, int d)
+{
+    if (field != BG_FIELD_FP31 && field != BG_FIELD_C128 && field != BG_FIELD_FPMONT) return BG_ERR_ARG;
+    if (metric != BG_METRIC_MOSTLY_MINUS && metric != BG_METRIC_ALTERNATING) return BG_ERR_ARG;
     if (n < 4 || n > 16 || d < 4 || d > 16) return BG_ERR_ARG;
     return BG_OK;
 }
 
-int make_plan(int field, int n, int d, LaunchPlan* plan)
+// default selection, cached: [field][metric][multi_state][n][d]
+Launch g_cache[3][2][2][17][17];
+std::atomic<unsigned char> g_cache_state[3][2][2][17][17];      // 0 empty, 1 ready, 2 unsupported
+std::mutex g_cache_mutex;
+// selection under an override: rebuilt when the override changes (measurement path, not hot)
+Launch g_over;
+int g_over_key[7] = {-2, 0, 0, 0, 0, 0, 0};
+
+int select(int field, int metric, int n, int d, bool multi_state, Launch** out)
 {
-    int rc = check_shape(field, n, d);
-    if (rc != BG_OK) return rc;
-    const bg::RecordLayout lay = bg::make_layout(n, d, vec_width(field, d));
-    plan->elem_bytes = field == BG_FIELD_FP31 ? 4 : 16;
-    plan->stride = lay.stride;
-    const int per_point = lay.stride * plan->elem_bytes;
-    int t = kMaxSmemPerBlock / per_point;
-    if (t < 1) return BG_ERR_UNSUPPORTED;
-    if (t > 32) t = 32;
-    plan->threads = t;
-    plan->smem_bytes = t * per_point;
-    plan->func = field == BG_FIELD_FP31 ? pick<Fp31>(n, d, &plan->specialised)
-                                        : pick<C128>(n, d, &plan->specialised);
-    return plan->func ? BG_OK : BG_ERR_UNSUPPORTED;
+    const int ok = g_override_kind.load(std::memory_order_relaxed), ow = g_override_w.load(std::memory_order_relaxed);
+    if (ok >= 0) {
+        std::lock_guard<std::mutex> lock(g_cache_mutex);
+        const int key[7] = {ok, ow, field, metric, n, d, (int)multi_state};
+        if (memcmp(key, g_over_key, sizeof(key)) != 0) {
+            g_over.attr_done = 0;
+            const KernelEntry* e = ok == 0 ? nullptr
+                                           : find_entry(field, metric, n, d, multi_state, ok - 1, ow);
+            int rc = BG_OK;
+            if (e) fill_entry(*e, &g_over);
+            else if (ok == 0 || !(e = find_entry(field, metric, n, d, multi_state, -1, 0)))
+                rc = fill_general(field, metric, n, d, &g_over);
+            else fill_entry(*e, &g_over);
+            if (rc != BG_OK) { g_over_key[0] = -2; return rc; }
+            memcpy(g_over_key, key, sizeof(key));
+        }
+        *out = &g_over;
+        return BG_OK;
+    }
+    Launch* L = &g_cache[field][metric][multi_state][n][d];
+    std::atomic<unsigned char>& st = g_cache_state[field][metric][multi_state][n][d];
+    unsigned char s = st.load(std::memory_order_acquire);
+    if (s == 0) {
+        std::lock_guard<std::mutex> lock(g_cache_mutex);
+        s = st.load(std::memory_order_relaxed);
+        if (s == 0) {
+            int rc = BG_OK;
+            if (const KernelEntry* e = find_entry(field, metric, n, d, multi_state, -1, 0)) fill_entry(*e, L);
+            else rc = fill_general(field, metric, n, d, L);
+            s = rc == BG_OK ? 1 : 2;
+            st.store(s, std::memory_order_release);
+        }
+    }
+    if (s != 1) return BG_ERR_UNSUPPORTED;
+    *out = L;
+    return BG_OK;
+}
+
+int ensure_attr(Launch* L)
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) { cudaGetLastError(); return BG_ERR_CUDA; }
+    const uint64_t bit = 1ull << dev;
+    if (L->attr_done.load(std::memory_order_acquire) & bit) return BG_OK;
+    if (cudaFuncSetAttribute(L->func, cudaFuncAttributeMaxDynamicSharedMemorySize, L->smem) != cudaSuccess) {
+        cudaGetLastError();
+        return BG_ERR_CUDA;
+    }
+    L->attr_done.fetch_or(bit, std::memory_order_release);
+    return BG_OK;
+}
+
+// ---- Montgomery constants of a prime ------------------------------------------------------------------
+bool mont_constants(uint32_t p, int i, FpMont::Params* q)
+{
+    if (!(p & 1u) || p <= (1u << 30) || p >= (1u << 31)) return false;
+    uint32_t inv = p;                                  // Newton: inv = p^-1 mod 2^32 (p odd; 3 bits correct at start)
+    for (int k = 0; k < 5; ++k) inv *= 2u - p * inv;
+    const uint64_t r = ((uint64_t)1 << 32) % p;
+    q->p[i] = p;
+    q->pinv[i] = 0u - inv;
+    q->one[i] = (uint32_t)r;
+    q->r2[i] = (uint32_t)(r * r % p);
+    q->half[i] = (uint32_t)(r * ((p + 1u) / 2u) % p);
+    return true;
 }
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
-template <class E>
-int launch_typed(const LaunchPlan& plan, int n, int64_t batch, const void* mom, const void* pol,
-                 void* out, void* cur, uint32_t* status, cudaStream_t stream)
+template <class F>
+int launch_typed(Launch* L, const bg_problem_t& pb, const typename F::Params& fld, int64_t batch, const void* mom,
+                 const void* pol, void* out, void* cur, uint32_t* status, cudaStream_t stream)
 {
-    KernelParams<E> prm;
+    typedef typename F::E E;
+    BgParams<F> prm;
     prm.mom = static_cast<const E*>(mom);
     prm.pol = static_cast<const E*>(pol);
     prm.out = static_cast<E*>(out);
     prm.currents = static_cast<E*>(cur);
     prm.status = status;
     prm.batch = batch;
-    prm.n = n;
-    prm.stride = plan.stride;
-    if (cudaFuncSetAttribute(plan.func, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.smem_bytes) !=
-        cudaSuccess) {
-        cudaGetLastError();
-        return BG_ERR_CUDA;
-    }
-    const int64_t blocks = (batch + plan.threads - 1) / plan.threads;
+    prm.states = pb.states;
+    prm.n = pb.n;
+    prm.stride = L->stride;
+    prm.fld = fld;
+    int rc = ensure_attr(L);
+    if (rc != BG_OK) return rc;
+    const int64_t blocks = (batch + L->points_per_block - 1) / L->points_per_block;
     if (blocks > 0x7fffffffLL) return BG_ERR_ARG;
+    const unsigned gy = pb.field == BG_FIELD_FPMONT ? (unsigned)pb.n_primes : 1u;
     void* args[] = {&prm};
-    if (cudaLaunchKernel(plan.func, dim3((unsigned)blocks), dim3(plan.threads), args, plan.smem_bytes,
-                         stream) != cudaSuccess) {
+    if (cudaLaunchKernel(L->func, dim3((unsigned)blocks, gy), dim3(L->threads), args, L->smem, stream) != cudaSuccess) {
         cudaGetLastError();
         return BG_ERR_CUDA;
     }
     return BG_OK;
 }
 
-template <class E>
-int launch_sweep(const SweepEntry& e, int64_t batch, const void* mom, const void* pol, void* out, void* cur,
-                 uint32_t* status, cudaStream_t stream)
+int check_problem(const bg_problem_t* pb)
 {
-    bg::TileParams<E> prm;
-    prm.mom = static_cast<const E*>(mom);
-    prm.pol = static_cast<const E*>(pol);
-    prm.out = static_cast<E*>(out);
-    prm.currents = static_cast<E*>(cur);
-    prm.status = status;
-    prm.batch = batch;
-    if (cudaFuncSetAttribute(e.func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)e.smem) != cudaSuccess) {
-        cudaGetLastError();
-        return BG_ERR_CUDA;
-    }
-    const int64_t blocks = (batch + e.tp - 1) / e.tp;
-    if (blocks > 0x7fffffffLL) return BG_ERR_ARG;
-    void* args[] = {&prm};
-    if (cudaLaunchKernel(e.func, dim3((unsigned)blocks), dim3(32 * e.w), args, e.smem, stream) != cudaSuccess) {
-        cudaGetLastError();
-        return BG_ERR_CUDA;
+    if (!pb) return BG_ERR_ARG;
+    int rc = check_shape(pb->field, pb->metric, pb->n, pb->d);
+    if (rc != BG_OK) return rc;
+    if (pb->states < 1 || pb->states > 65535) return BG_ERR_ARG;
+    if (pb->field == BG_FIELD_FPMONT) {
+        if (pb->n_primes < 1 || pb->n_primes > BG_MAX_PRIMES) return BG_ERR_ARG;
+    } else if (pb->n_primes != 0) {
+        return BG_ERR_ARG;
     }
     return BG_OK;
 }
 
-int run(int field, int n, int d, int64_t batch, const void* mom, const void* pol, void* out, void* cur,
+int run(const bg_problem_t& pb, int64_t batch, const void* mom, const void* pol, void* out, void* cur,
         uint32_t* status, cudaStream_t stream)
 {
-    LaunchPlan plan;
-    int rc = make_plan(field, n, d, &plan);
+    int rc = check_problem(&pb);
+    if (rc != BG_OK) return rc;
+    FpMont::Params mont{};
+    if (pb.field == BG_FIELD_FPMONT)
+        for (int i = 0; i < pb.n_primes; ++i)
+            if (!mont_constants(pb.primes[i], i, &mont)) return BG_ERR_ARG;
+    Launch* L = nullptr;
+    rc = select(pb.field, pb.metric, pb.n, pb.d, pb.states > 1, &L);
     if (rc != BG_OK) return rc;
     if (batch < 0) return BG_ERR_ARG;
     if (batch == 0) return BG_OK;
@@ -229,13 +270,20 @@ int run(int field, int n, int d, int64_t batch, const void* mom, const void* pol
         (reinterpret_cast<uintptr_t>(status) & 3u))
         return BG_ERR_ARG;
     if (out == mom || out == pol) return BG_ERR_ARG;
-    if (const SweepEntry* e = find_sweep(field, n, d)) {
-        if (field == BG_FIELD_FP31) return launch_sweep<uint32_t>(*e, batch, mom, pol, out, cur, status, stream);
-        return launch_sweep<double2>(*e, batch, mom, pol, out, cur, status, stream);
+    if (cur && (pb.states != 1 || pb.n_primes > 1)) return BG_ERR_ARG;
+    switch (pb.field) {
+        case BG_FIELD_FP31: return launch_typed<Fp31>(L, pb, Fp31::Params{}, batch, mom, pol, out, cur, status, stream);
+        case BG_FIELD_C128: return launch_typed<C128>(L, pb, C128::Params{}, batch, mom, pol, out, cur, status, stream);
+        default: return launch_typed<FpMont>(L, pb, mont, batch, mom, pol, out, cur, status, stream);
     }
-    if (field == BG_FIELD_FP31)
-        return launch_typed<uint32_t>(plan, n, batch, mom, pol, out, cur, status, stream);
-    return launch_typed<double2>(plan, n, batch, mom, pol, out, cur, status, stream);
+}
+
+bg_problem_t simple_problem(int field, int metric, int n, int d, int states)
+{
+    bg_problem_t pb;
+    memset(&pb, 0, sizeof(pb));
+    pb.field = field; pb.metric = metric; pb.n = n; pb.d = d; pb.states = states;
+    return pb;
 }
 
 int64_t binom(int n, int k)
@@ -248,6 +296,31 @@ int64_t binom(int n, int k)
 
 size_t round256(size_t x) { return (x + 255) & ~(size_t)255; }
 
+// two persistent streams per device for bg_amplitudes_host, created on first use and never destroyed
+cudaStream_t g_host_streams[kMaxDevices][2];
+std::atomic<bool> g_host_streams_ready[kMaxDevices];
+std::mutex g_host_mutex;
+
+int host_streams(cudaStream_t (&s)[2])
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) { cudaGetLastError(); return BG_ERR_CUDA; }
+    if (!g_host_streams_ready[dev].load(std::memory_order_acquire)) {
+        std::lock_guard<std::mutex> lock(g_host_mutex);
+        if (!g_host_streams_ready[dev].load(std::memory_order_relaxed)) {
+            for (int i = 0; i < 2; ++i)
+                if (cudaStreamCreateWithFlags(&g_host_streams[dev][i], cudaStreamNonBlocking) != cudaSuccess) {
+                    cudaGetLastError();
+                    return BG_ERR_CUDA;
+                }
+            g_host_streams_ready[dev].store(true, std::memory_order_release);
+        }
+    }
+    s[0] = g_host_streams[dev][0];
+    s[1] = g_host_streams[dev][1];
+    return BG_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -255,25 +328,65 @@ extern "C" {
 int bg_amplitudes(int field, int n, int d, int64_t batch, const void* momenta, const void* polarisations,
                   void* out, cudaStream_t stream)
 {
-    return run(field, n, d, batch, momenta, polarisations, out, nullptr, nullptr, stream);
+    if (field == BG_FIELD_FPMONT) return BG_ERR_ARG;          // needs a prime: bg_amplitudes_primes / bg_evaluate
+    return run(simple_problem(field, BG_METRIC_MOSTLY_MINUS, n, d, 1), batch, momenta, polarisations, out, nullptr,
+               nullptr, stream);
 }
 
 int bg_amplitudes_status(int field, int n, int d, int64_t batch, const void* momenta,
                          const void* polarisations, void* out, uint32_t* status, cudaStream_t stream)
 {
-    return run(field, n, d, batch, momenta, polarisations, out, nullptr, status, stream);
+    if (field == BG_FIELD_FPMONT) return BG_ERR_ARG;
+    return run(simple_problem(field, BG_METRIC_MOSTLY_MINUS, n, d, 1), batch, momenta, polarisations, out, nullptr,
+               status, stream);
 }
 
 int bg_currents(int field, int n, int d, int64_t batch, const void* momenta, const void* polarisations,
                 void* out, void* currents, uint32_t* status, cudaStream_t stream)
 {
-    return run(field, n, d, batch, momenta, polarisations, out, currents, status, stream);
+    if (field == BG_FIELD_FPMONT) return BG_ERR_ARG;
+    return run(simple_problem(field, BG_METRIC_MOSTLY_MINUS, n, d, 1), batch, momenta, polarisations, out, currents,
+               status, stream);
+}
+
+int bg_evaluate(const bg_problem_t* problem, int64_t batch, const void* momenta, const void* polarisations,
+                void* out, void* currents, uint32_t* status, cudaStream_t stream)
+{
+    if (!problem) return BG_ERR_ARG;
+    return run(*problem, batch, momenta, polarisations, out, currents, status, stream);
+}
+
+int bg_amplitudes_states(int field, int n, int d, int64_t batch, int states, const void* momenta,
+                         const void* polarisations, void* out, uint32_t* status, cudaStream_t stream)
+{
+    if (field == BG_FIELD_FPMONT) return BG_ERR_ARG;
+    return run(simple_problem(field, BG_METRIC_MOSTLY_MINUS, n, d, states), batch, momenta, polarisations, out,
+               nullptr, status, stream);
+}
+
+int bg_amplitudes_primes(int metric, int n, int d, int64_t batch, int n_primes, const uint32_t* primes,
+                         const void* momenta, const void* polarisations, void* out, uint32_t* status,
+                         cudaStream_t stream)
+{
+    if (!primes || n_primes < 1 || n_primes > BG_MAX_PRIMES) return BG_ERR_ARG;
+    bg_problem_t pb = simple_problem(BG_FIELD_FPMONT, metric, n, d, 1);
+    pb.n_primes = n_primes;
+    for (int i = 0; i < n_primes; ++i) pb.primes[i] = primes[i];
+    return run(pb, batch, momenta, polarisations, out, nullptr, status, stream);
+}
+
+int bg_set_kernel_override(int kind, int warps)
+{
+    g_override_kind = kind < 0 || kind > 3 ? -1 : kind;
+    g_override_w = warps < 0 ? 0 : warps;
+    return BG_OK;
 }
 
 size_t bg_host_workspace_bytes(int field, int n, int d, int64_t chunk_points)
 {
-    if (check_shape(field, n, d) != BG_OK || chunk_points <= 0) return 0;
-    const size_t w = field == BG_FIELD_FP31 ? 4 : 16;
+    if (check_shape(field, BG_METRIC_MOSTLY_MINUS, n, d) != BG_OK || field == BG_FIELD_FPMONT || chunk_points <= 0)
+        return 0;
+    const size_t w = elem_bytes(field);
     const size_t in = round256((size_t)chunk_points * n * d * w);
     const size_t o = round256((size_t)chunk_points * w);
     const size_t st = round256((size_t)chunk_points * 4);
@@ -284,8 +397,9 @@ int bg_amplitudes_host(int field, int n, int d, int64_t batch, const void* host_
                        const void* host_polarisations, void* host_out, uint32_t* host_status,
                        void* workspace, size_t workspace_bytes)
 {
-    LaunchPlan plan;
-    int rc = make_plan(field, n, d, &plan);
+    if (field == BG_FIELD_FPMONT) return BG_ERR_ARG;
+    const bg_problem_t pb = simple_problem(field, BG_METRIC_MOSTLY_MINUS, n, d, 1);
+    int rc = check_problem(&pb);
     if (rc != BG_OK) return rc;
     if (batch < 0) return BG_ERR_ARG;
     if (batch == 0) return BG_OK;
@@ -298,20 +412,15 @@ int bg_amplitudes_host(int field, int n, int d, int64_t batch, const void* host_
         if (c >= batch) break;
     }
     if (chunk == 0) return BG_ERR_ARG;
-    const size_t w = field == BG_FIELD_FP31 ? 4 : 16;
+    const size_t w = elem_bytes(field);
     const size_t in_b = round256((size_t)chunk * n * d * w);
     const size_t out_b = round256((size_t)chunk * w);
     const size_t st_b = round256((size_t)chunk * 4);
     const size_t slot_b = 2 * in_b + out_b + st_b;
 
-    cudaStream_t s[2] = {nullptr, nullptr};
-    for (int i = 0; i < 2; ++i)
-        if (cudaStreamCreateWithFlags(&s[i], cudaStreamNonBlocking) != cudaSuccess) {
-            cudaGetLastError();
-            if (s[0]) cudaStreamDestroy(s[0]);
-            return BG_ERR_CUDA;
-        }
-    rc = BG_OK;
+    cudaStream_t s[2];
+    rc = host_streams(s);
+    if (rc != BG_OK) return rc;
     int64_t done = 0;
     for (int c = 0; done < batch && rc == BG_OK; ++c, done += chunk) {
         const int64_t nb = batch - done < chunk ? batch - done : chunk;
@@ -329,7 +438,7 @@ int bg_amplitudes_host(int field, int n, int d, int64_t batch, const void* host_
             e = cudaMemcpyAsync(dp, static_cast<const unsigned char*>(host_polarisations) + off_in,
                                 nbytes, cudaMemcpyHostToDevice, st);
         if (e != cudaSuccess) { rc = BG_ERR_CUDA; break; }
-        rc = run(field, n, d, nb, dm, dp, dout, nullptr, host_status ? dst : nullptr, st);
+        rc = run(pb, nb, dm, dp, dout, nullptr, host_status ? dst : nullptr, st);
         if (rc != BG_OK) break;
         e = cudaMemcpyAsync(static_cast<unsigned char*>(host_out) + (size_t)done * w, dout, (size_t)nb * w,
                             cudaMemcpyDeviceToHost, st);
@@ -337,10 +446,8 @@ int bg_amplitudes_host(int field, int n, int d, int64_t batch, const void* host_
             e = cudaMemcpyAsync(host_status + done, dst, (size_t)nb * 4, cudaMemcpyDeviceToHost, st);
         if (e != cudaSuccess) { rc = BG_ERR_CUDA; break; }
     }
-    for (int i = 0; i < 2; ++i) {
+    for (int i = 0; i < 2; ++i)
         if (cudaStreamSynchronize(s[i]) != cudaSuccess) rc = BG_ERR_CUDA;
-        cudaStreamDestroy(s[i]);
-    }
     if (rc == BG_ERR_CUDA) cudaGetLastError();
     return rc;
 }
@@ -358,14 +465,14 @@ const char* bg_status_string(int status)
     return "unknown status";
 }
 
-const char* bg_version(void) { return "bg_b200 0.1 (sm_100a)"; }
+const char* bg_version(void) { return "bg_b200 0.2 (sm_100a)"; }
 
 int bg_op_count(int field, int n, int d, bg_opcount_t* out)
 {
-    if (check_shape(field, n, d) != BG_OK || !out) return BG_ERR_ARG;
+    if (check_shape(field, BG_METRIC_MOSTLY_MINUS, n, d) != BG_OK || !out) return BG_ERR_ARG;
     const int m = n - 1;
     const int64_t R = (int64_t)m * (m - 1) / 2 - 1;
-    const int64_t w = field == BG_FIELD_FP31 ? 4 : 16;
+    const int64_t w = elem_bytes(field);
     out->currents = (int64_t)n * (n - 1) / 2;
     out->propagators = R;
     out->splits3 = binom(n, 3);
@@ -374,46 +481,47 @@ int bg_op_count(int field, int n, int d, bg_opcount_t* out)
     out->mul_v4 = 6 * d * out->splits4;
     out->mul_other = d * R + 3 * (R - 1) + d * R + d;
     out->mul_ref = out->mul_v3 + out->mul_v4 + out->mul_other;
-    // kernel: per 3-split 3 dots + 4 axpys, per 4-split 1 dot + 1 axpy, invariants, propagators,
-    // Montgomery trick, final contraction
-    out->mul_factored = 7 * d * out->splits3 + 2 * d * out->splits4 + d * R + 3 * (R - 1) + d * R + d;
+    // what the kernels' factored form executes (bg.h): per 3-split 3 dots + 3 axpys, per 4-split 1 dot + 1
+    // axpy; per multi-gluon current (R + 1 of them) the boundary term (d), sum_k h_k / 2 (1) and, unless
+    // top, the propagator (d) and 2 P.J (d); the final contraction (d); single-gluon 2 k.eps (m d);
+    // invariants (d R) and the batch inverse (3 (R-1) + 38 for the inversion chain)
+    out->mul_factored = 6 * d * out->splits3 + 2 * d * out->splits4 + (R + 1) * (d + 1) + 2 * d * R + d +
+                        (int64_t)m * d + d * R + 3 * (R - 1) + 38;
     out->bytes_in = 2 * (int64_t)n * d * w;
     out->bytes_out = w;
     return BG_OK;
 }
 
-int bg_kernel_info(int field, int n, int d, bg_kernel_info_t* out)
+int bg_kernel_info_problem(const bg_problem_t* problem, bg_kernel_info_t* out)
 {
     if (!out) return BG_ERR_ARG;
-    LaunchPlan plan;
-    int rc = make_plan(field, n, d, &plan);
+    int rc = check_problem(problem);
     if (rc != BG_OK) return rc;
-    const void* func = plan.func;
-    if (const SweepEntry* e = find_sweep(field, n, d)) {
-        // the compile-time (n, d) fast path: one tile of 32 points per block, e->w warps
-        out->specialised = 1 + e->kind;          // 1: bg_tile_kernel, 2: bg_level_kernel, 3: bg_split_kernel
-        out->threads_per_block = 32 * e->w;
-        out->points_per_block = e->tp;
-        out->smem_bytes_per_block = (int)e->smem;
-        out->smem_bytes_per_point = (int)(e->smem / e->tp);
-        func = e->func;
-    } else {
-        out->specialised = 0;
-        out->threads_per_block = plan.threads;
-        out->points_per_block = plan.threads;
-        out->smem_bytes_per_block = plan.smem_bytes;
-        out->smem_bytes_per_point = plan.stride * plan.elem_bytes;
-    }
+    Launch* L = nullptr;
+    rc = select(problem->field, problem->metric, problem->n, problem->d, problem->states > 1, &L);
+    if (rc != BG_OK) return rc;
+    out->specialised = L->kind == BG_KIND_GENERAL ? 0 : 1 + L->kind;
+    out->threads_per_block = L->threads;
+    out->points_per_block = L->points_per_block;
+    out->smem_bytes_per_block = L->smem;
+    out->smem_bytes_per_point = L->smem / L->points_per_block;
     int bps = kSmemPerSm / (out->smem_bytes_per_block + kSmemReservedPerBlock);
     out->blocks_per_sm = bps > 32 ? 32 : bps;
     cudaFuncAttributes attr;
-    if (cudaFuncGetAttributes(&attr, func) == cudaSuccess) {
+    if (cudaFuncGetAttributes(&attr, L->func) == cudaSuccess) {
         out->regs_per_thread = attr.numRegs;
     } else {
         cudaGetLastError();
         out->regs_per_thread = -1;
     }
     return BG_OK;
+}
+
+int bg_kernel_info(int field, int n, int d, bg_kernel_info_t* out)
+{
+    bg_problem_t pb = simple_problem(field, BG_METRIC_MOSTLY_MINUS, n, d, 1);
+    if (field == BG_FIELD_FPMONT) { pb.n_primes = 1; pb.primes[0] = 2147483629u; }
+    return bg_kernel_info_problem(&pb, out);
 }
 
 }  // extern "C"

@@ -1,0 +1,152 @@
+// bg_common.cuh -- pieces shared by every Berends-Giele kernel: launch parameters, vector
+// load/store, Minkowski products with a compile-time metric, lane-pair sums.
+//
+// Algebra used by all kernels ("factored form" of the i-free V3, V4 of Eq.(7), PAPER.md:99-101;
+// DESIGN.md §6).  For the current (i..j) with own momentum X = P_{i,j} and a split
+// A = J(i..k), B = J(k+1..j), with PS2_c = 2 (k_1+..+k_c) (Eq.(7)) and the
+// per-current scalars U = 2 P.J + S, V = 2 P.J - S (P the current's own momentum,
+// S(i..l) = sum_k J(i..k).J(k+1..l)):
+//
+//   bracket^mu = sum_k [ h_k PS2_k^mu + (2X.A - U_A) B^mu + (V_B - 2X.B) A^mu ]
+//              - (sum_k h_k)/2 (PS2_{i-1} + PS2_j)^mu
+//              + sum_{k<l} 2 (A_k . C_l) J(k+1..l)^mu ,        h_k = A.B
+//
+// Per 3-split 3 dot products + 3 axpys, per 4-split 1 dot + 1 axpy.  Exact over F_p, hence
+// bit-identical to the literal evaluation; over complex128 a reordering within DESIGN.md R9/R10.
+#pragma once
+#include "bg_field.cuh"
+
+namespace bg {
+
+// Launch parameters of every recursion kernel.  blockIdx.y = index of the prime of a
+// multi-prime call (0 otherwise): all arrays of prime q start q * (their size) elements in.
+template <class F>
+struct BgParams {
+    typedef typename F::E E;
+    const E* mom;         // [primes][batch][n][D]
+    const E* pol;         // [primes][batch][states][n][D]
+    E* out;               // [primes][batch][states]
+    E* currents;          // NULL or [batch][m][m][D]   (states == 1, one prime)
+    uint32_t* status;     // NULL or [primes][batch]
+    long long batch;
+    int states;           // S >= 1 polarisation configurations per momentum point (Eq.(4))
+    int n;                // general kernel only
+    int stride;           // general kernel only: record stride in elements
+    typename F::Params fld;
+};
+
+template <class F, int D> struct VecWidth { static constexpr int value = 1; };
+template <int D> struct VecWidth<Fp31, D> { static constexpr int value = (D % 4 == 0) ? 4 : (D % 2 == 0) ? 2 : 1; };
+template <int D> struct VecWidth<FpMont, D> { static constexpr int value = VecWidth<Fp31, D>::value; };
+
+// the memory type of one vector unit of U elements, and the input conversion applied to it
+template <class F, int U> struct VecType { typedef typename F::E type; };
+template <> struct VecType<Fp31, 2> { typedef uint2 type; };
+template <> struct VecType<Fp31, 4> { typedef uint4 type; };
+template <> struct VecType<FpMont, 2> { typedef uint2 type; };
+template <> struct VecType<FpMont, 4> { typedef uint4 type; };
+template <class F> __device__ __forceinline__ typename F::E load_unit(const F& f, typename F::E v) { return f.load_input(v); }
+template <class F> __device__ __forceinline__ uint2 load_unit(const F& f, uint2 v)
+{
+    return make_uint2(f.load_input(v.x), f.load_input(v.y));
+}
+template <class F> __device__ __forceinline__ uint4 load_unit(const F& f, uint4 v)
+{
+    return make_uint4(f.load_input(v.x), f.load_input(v.y), f.load_input(v.z), f.load_input(v.w));
+}
+
+template <class F, int D>
+__device__ __forceinline__ void ld_vec(const typename F::E* p, typename F::E (&v)[D])
+{
+    constexpr int W = VecWidth<F, D>::value;
+    if constexpr (W == 4) {
+#pragma unroll
+        for (int q = 0; q < D / 4; ++q) {
+            uint4 t = reinterpret_cast<const uint4*>(p)[q];
+            v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
+        }
+    } else if constexpr (W == 2) {
+#pragma unroll
+        for (int q = 0; q < D / 2; ++q) {
+            uint2 t = reinterpret_cast<const uint2*>(p)[q];
+            v[2 * q] = t.x; v[2 * q + 1] = t.y;
+        }
+    } else {
+#pragma unroll
+        for (int q = 0; q < D; ++q) v[q] = p[q];
+    }
+}
+
+template <class F, int D>
+__device__ __forceinline__ void st_vec(typename F::E* p, const typename F::E (&v)[D])
+{
+    constexpr int W = VecWidth<F, D>::value;
+    if constexpr (W == 4) {
+#pragma unroll
+        for (int q = 0; q < D / 4; ++q)
+            reinterpret_cast<uint4*>(p)[q] = make_uint4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+    } else if constexpr (W == 2) {
+#pragma unroll
+        for (int q = 0; q < D / 2; ++q) reinterpret_cast<uint2*>(p)[q] = make_uint2(v[2 * q], v[2 * q + 1]);
+    } else {
+#pragma unroll
+        for (int q = 0; q < D; ++q) p[q] = v[q];
+    }
+}
+
+// sum_mu x_mu y_mu, plain (the metric is already inside one operand); headroom by relief (one
+// operand of every product is a canonical residue <= p-1: stored vectors always are)
+template <class F, int D>
+__device__ __forceinline__ typename F::A dot_plain(const F& f, const typename F::E (&x)[D],
+                                                    const typename F::E (&y)[D])
+{
+    typename F::A s = f.zero();
+#pragma unroll
+    for (int mu = 0; mu < D; ++mu) {
+        if (mu >= F::kCap0 && ((mu - F::kCap0) % F::kCapR) == 0) s = f.relief(s);
+        s = f.mad(x[mu], y[mu], s);
+    }
+    return s;
+}
+
+// x or -x (flag usually folds at compile time)
+__device__ __forceinline__ uint32_t cneg(const Fp31&, uint32_t x, bool flag) { return x ^ (flag ? kP : 0u); }
+__device__ __forceinline__ uint32_t cneg(const FpMont& f, uint32_t x, bool flag) { return flag ? f.p - x : x; }
+__device__ __forceinline__ double2 cneg(const C128&, double2 x, bool flag)
+{
+    return flag ? make_double2(-x.x, -x.y) : x;
+}
+
+// nx_mu = -g_{mu mu} x_mu for the components mu0 .. mu0+DL-1 a lane owns, so that
+// dot_plain(nx, y) = MINUS the Minkowski product x.y (restricted to those components)
+template <class F, int MET, int DL>
+__device__ __forceinline__ void lower_neg(const F& f, int mu0, const typename F::E (&x)[DL], typename F::E (&nx)[DL])
+{
+#pragma unroll
+    for (int mu = 0; mu < DL; ++mu) nx[mu] = cneg(f, x[mu], !Metric<MET>::minus(mu0 + mu));
+}
+
+// x2_mu = g_{mu mu} (h - l)_mu : twice the covariant P_{i,j} from the doubled prefix sums
+template <class F, int MET, int DL>
+__device__ __forceinline__ void lower_diff(const F& f, int mu0, const typename F::E (&h)[DL],
+                                           const typename F::E (&l)[DL], typename F::E (&x2)[DL])
+{
+#pragma unroll
+    for (int mu = 0; mu < DL; ++mu) x2[mu] = cneg(f, f.sub(h[mu], l[mu]), Metric<MET>::minus(mu0 + mu));
+}
+
+// value summed over the S lanes that share a point (lanes l and l + TP of a warp when S == 2)
+template <class F, int S, int TP>
+__device__ __forceinline__ uint32_t lane_sum(const F& f, uint32_t x)
+{
+    if constexpr (S == 1) return x;
+    else return f.add(x, __shfl_xor_sync(0xffffffffu, x, TP));
+}
+template <class F, int S, int TP>
+__device__ __forceinline__ double2 lane_sum(const F&, double2 x)
+{
+    if constexpr (S == 1) return x;
+    else return make_double2(x.x + __shfl_xor_sync(0xffffffffu, x.x, TP), x.y + __shfl_xor_sync(0xffffffffu, x.y, TP));
+}
+
+}  // namespace bg

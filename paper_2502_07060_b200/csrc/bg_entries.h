@@ -1,27 +1,35 @@
-// bg_entries.h -- the table of compile-time (n, d) kernel instances, shared between bg_api.cu (which
-// selects and launches) and the bg_inst_*.cu translation units (which instantiate the kernels).
+// bg_entries.h -- the table of compile-time (field, metric, n, d) kernel instances, shared between
+// bg_api.cu (which selects and launches) and the bg_inst_*.cu translation units (which instantiate
+// the kernels; several units because the work lists of an instance sit in constant memory, a module
+// has 64 KB of it, and nvcc compiles them in parallel).
 #pragma once
 #include <stddef.h>
 
-struct SweepEntry {
-    int field, n, d, w;      // w: warps per tile (bg_reg_kernel: independent warps per block)
-    int kind;                // 0: bg_tile_kernel (table-driven loop over splittings), 1: bg_level_kernel (levels
-                             // unrolled), 2: bg_split_kernel (table-driven, two lanes per point), 3: bg_reg_kernel
-                             // (currents in registers, no barriers), 4: bg_unit_kernel (one body per number of
-                             // 4-gluon splits)
+enum BgKernelKind {
+    BG_KIND_UNIT1 = 0,       // bg_unit_kernel, one lane per point, 32-point tiles
+    BG_KIND_UNIT2 = 1,       // bg_unit_kernel, two lanes per point, 16-point tiles
+    BG_KIND_REG = 2,         // bg_reg_kernel: currents in registers, no barriers (one state configuration only)
+    BG_KIND_GENERAL = 3      // bg_general_kernel: run-time n, one thread per point (not in the tables)
+};
+
+struct KernelEntry {
+    int field, metric, n, d;
+    int w;                   // warps per tile (bg_reg_kernel: independent warps per block)
+    int kind;                // BgKernelKind
     int tp;                  // points per block
     const void* func;
     size_t smem;
 };
 
-// first entry of a shape = the default; the others are selected with the tuning knobs BG_KERNEL
-// (tile|level|split|reg|unit) and BG_SWEEP_W (warps per tile), read from the environment per call
-const SweepEntry* bg_entries_default(int* count);     // bg_inst_default.cu
-const SweepEntry* bg_entries_fp_alt(int* count);      // bg_inst_fp_alt.cu
-const SweepEntry* bg_entries_c128_alt(int* count);    // bg_inst_c128_alt.cu
-const SweepEntry* bg_entries_paper(int* count);       // bg_inst_paper.cu
-const SweepEntry* bg_entries_grid0(int* count);       // bg_inst_grid0.cu
-const SweepEntry* bg_entries_grid1(int* count);       // bg_inst_grid1.cu
-const SweepEntry* bg_entries_grid2(int* count);       // bg_inst_grid2.cu
-const SweepEntry* bg_entries_cgrid0(int* count);      // bg_inst_cgrid0.cu
-const SweepEntry* bg_entries_cgrid1(int* count);      // bg_inst_cgrid1.cu
+// first entry of a shape = the default; the others are reachable through bg_set_kernel_override
+#define BG_ENTRY_TABLES(X) X(default) X(fp_alt) X(c128_alt) X(paper) X(grid0) X(grid1) X(grid2) X(cgrid0) X(cgrid1) \
+    X(metric) X(mont)
+#define BG_DECLARE_TABLE(name) const KernelEntry* bg_entries_##name(int* count);
+BG_ENTRY_TABLES(BG_DECLARE_TABLE)
+#undef BG_DECLARE_TABLE
+
+// bg_general_kernel<F, MET, D> for d = 4..16, one translation unit per field (bg_inst_general_*.cu);
+// NULL if (metric, d) is out of range
+const void* bg_general_kernel_ptr_fp31(int metric, int d);
+const void* bg_general_kernel_ptr_c128(int metric, int d);
+const void* bg_general_kernel_ptr_mont(int metric, int d);

@@ -1,16 +1,10 @@
-// bg_inst_c128_alt.cu -- alternative complex128 instances for A/B runs (BG_KERNEL, BG_SWEEP_W)
+// bg_inst_c128_alt.cu -- alternative complex128 instances for A/B runs (bg_set_kernel_override)
 #include "bg_inst_common.cuh"
 
-const SweepEntry* bg_entries_c128_alt(int* count)
-{
-    static const SweepEntry table[] = {
-        level_entry<C128, 6, 4, 2>(BG_FIELD_C128),
-        level_entry<C128, 6, 4, 4>(BG_FIELD_C128),
-        sweep_entry<C128, 6, 4, 4>(BG_FIELD_C128),
-        sweep_entry<C128, 6, 4, 2>(BG_FIELD_C128),
-        split_entry<C128, 6, 4, 2>(BG_FIELD_C128),
-        split_entry<C128, 6, 4, 4>(BG_FIELD_C128),
-    };
-    *count = (int)(sizeof(table) / sizeof(table[0]));
-    return table;
-}
+BG_DEFINE_TABLE(c128_alt,
+    unit_entry<C128, MM, 6, 4, 2, 2>(),       // also the cfg1 shape with several state configurations
+    unit_entry<C128, MM, 6, 4, 4, 2>(),
+    unit_entry<C128, MM, 6, 4, 2, 1>(),
+    unit_entry<C128, MM, 6, 4, 4, 1>(),
+    unit_entry<C128, MM, 12, 6, 8, 2>(),
+)

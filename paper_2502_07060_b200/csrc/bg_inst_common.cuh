@@ -2,46 +2,37 @@
 #pragma once
 #include "../../include/bg.h"
 #include "bg_entries.h"
-#include "bg_level.cuh"
 #include "bg_reg.cuh"
-#include "bg_split.cuh"
-#include "bg_tile.cuh"
 #include "bg_unit.cuh"
 
 namespace {
 
 using bg::C128;
 using bg::Fp31;
+using bg::FpMont;
+constexpr int MM = BG_METRIC_MOSTLY_MINUS, ALT = BG_METRIC_ALTERNATING;
 
-template <class F, int N, int D, int W>
-SweepEntry sweep_entry(int field)
+// bg_unit_kernel with S lanes per point and W warps per tile
+template <class F, int MET, int N, int D, int W, int S = 1>
+KernelEntry unit_entry()
 {
-    return SweepEntry{field, N, D, W, 0, 32, reinterpret_cast<const void*>(&bg::bg_tile_kernel<F, N, D, W>),
-                      bg::TileCfg<F, N, D, W>::SMEM_BYTES};
+    return KernelEntry{F::kFieldId, MET, N, D, W, S == 1 ? BG_KIND_UNIT1 : BG_KIND_UNIT2, 32 / S,
+                       reinterpret_cast<const void*>(&bg::bg_unit_kernel<F, MET, N, D, W, S>),
+                       bg::TileCfg<F, N, D, W, S>::SMEM_BYTES};
 }
-template <class F, int N, int D, int W>
-SweepEntry level_entry(int field)
+template <class F, int MET, int N, int D>
+KernelEntry reg_entry()
 {
-    return SweepEntry{field, N, D, W, 1, 32, reinterpret_cast<const void*>(&bg::bg_level_kernel<F, N, D, W>),
-                      bg::TileCfg<F, N, D, W>::SMEM_BYTES};
-}
-template <class F, int N, int D, int W>
-SweepEntry split_entry(int field)
-{
-    return SweepEntry{field, N, D, W, 2, 16, reinterpret_cast<const void*>(&bg::bg_split_kernel<F, N, D, W, 2>),
-                      bg::SplitCfg<F, N, D, W, 2>::SMEM_BYTES};
-}
-template <class F, int N, int D>
-SweepEntry reg_entry(int field)
-{
-    return SweepEntry{field, N, D, bg::RegCfg<F, N, D>::WARPS, 3, 16 * bg::RegCfg<F, N, D>::WARPS,
-                      reinterpret_cast<const void*>(&bg::bg_reg_kernel<F, N, D>), bg::RegCfg<F, N, D>::SMEM_BYTES};
-}
-template <class F, int N, int D, int W>
-SweepEntry unit_entry(int field)
-{
-    return SweepEntry{field, N, D, W, 4, 32, reinterpret_cast<const void*>(&bg::bg_unit_kernel<F, N, D, W>),
-                      bg::TileCfg<F, N, D, W>::SMEM_BYTES};
+    return KernelEntry{F::kFieldId, MET, N, D, bg::RegCfg<F, N, D>::WARPS, BG_KIND_REG, 16 * bg::RegCfg<F, N, D>::WARPS,
+                       reinterpret_cast<const void*>(&bg::bg_reg_kernel<F, MET, N, D>), bg::RegCfg<F, N, D>::SMEM_BYTES};
 }
 
 }  // namespace
+
+#define BG_DEFINE_TABLE(name, ...)                                              \
+    const KernelEntry* bg_entries_##name(int* count)                            \
+    {                                                                           \
+        static const KernelEntry table[] = {__VA_ARGS__};                       \
+        *count = (int)(sizeof(table) / sizeof(table[0]));                       \
+        return table;                                                           \
+    }

@@ -1,0 +1,8 @@
+// bg_inst_general_mont.cu -- the run-time-n kernel over FpMont, both metrics, d = 4..16
+#include "bg_inst_general.cuh"
+
+const void* bg_general_kernel_ptr_mont(int metric, int d)
+{
+    return metric == BG_METRIC_MOSTLY_MINUS ? general_for_d<bg::FpMont, BG_METRIC_MOSTLY_MINUS>(d)
+         : metric == BG_METRIC_ALTERNATING ? general_for_d<bg::FpMont, BG_METRIC_ALTERNATING>(d) : nullptr;
+}

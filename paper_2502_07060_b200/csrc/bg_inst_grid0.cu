@@ -3,20 +3,15 @@
 // the 64 KB of constant memory per module.
 #include "bg_inst_common.cuh"
 
-const SweepEntry* bg_entries_grid0(int* count)
-{
-    static const SweepEntry table[] = {
-        unit_entry<Fp31, 4, 5, 1>(BG_FIELD_FP31),
-        unit_entry<Fp31, 7, 5, 4>(BG_FIELD_FP31),
-        unit_entry<Fp31, 10, 5, 8>(BG_FIELD_FP31),
-        unit_entry<Fp31, 7, 6, 4>(BG_FIELD_FP31),
-        unit_entry<Fp31, 5, 7, 1>(BG_FIELD_FP31),
-        unit_entry<Fp31, 8, 7, 4>(BG_FIELD_FP31),
-        unit_entry<Fp31, 4, 9, 1>(BG_FIELD_FP31),
-        unit_entry<Fp31, 7, 9, 4>(BG_FIELD_FP31),
-        unit_entry<Fp31, 10, 9, 8>(BG_FIELD_FP31),
-        unit_entry<Fp31, 7, 10, 4>(BG_FIELD_FP31),
-    };
-    *count = (int)(sizeof(table) / sizeof(table[0]));
-    return table;
-}
+BG_DEFINE_TABLE(grid0,
+    unit_entry<Fp31, MM, 4, 5, 1>(),
+    unit_entry<Fp31, MM, 7, 5, 4>(),
+    unit_entry<Fp31, MM, 10, 5, 8>(),
+    unit_entry<Fp31, MM, 7, 6, 4>(),
+    unit_entry<Fp31, MM, 5, 7, 1>(),
+    unit_entry<Fp31, MM, 8, 7, 4>(),
+    unit_entry<Fp31, MM, 4, 9, 1>(),
+    unit_entry<Fp31, MM, 7, 9, 4>(),
+    unit_entry<Fp31, MM, 10, 9, 8>(),
+    unit_entry<Fp31, MM, 7, 10, 4>(),
+)

@@ -3,20 +3,15 @@
 // the 64 KB of constant memory per module.
 #include "bg_inst_common.cuh"
 
-const SweepEntry* bg_entries_grid1(int* count)
-{
-    static const SweepEntry table[] = {
-        unit_entry<Fp31, 5, 5, 1>(BG_FIELD_FP31),
-        unit_entry<Fp31, 8, 5, 4>(BG_FIELD_FP31),
-        unit_entry<Fp31, 4, 6, 1>(BG_FIELD_FP31),
-        unit_entry<Fp31, 10, 6, 8>(BG_FIELD_FP31),
-        unit_entry<Fp31, 6, 7, 2>(BG_FIELD_FP31),
-        unit_entry<Fp31, 9, 7, 4>(BG_FIELD_FP31),
-        unit_entry<Fp31, 5, 9, 1>(BG_FIELD_FP31),
-        unit_entry<Fp31, 8, 9, 4>(BG_FIELD_FP31),
-        unit_entry<Fp31, 4, 10, 1>(BG_FIELD_FP31),
-        unit_entry<Fp31, 8, 10, 4>(BG_FIELD_FP31),
-    };
-    *count = (int)(sizeof(table) / sizeof(table[0]));
-    return table;
-}
+BG_DEFINE_TABLE(grid1,
+    unit_entry<Fp31, MM, 5, 5, 1>(),
+    unit_entry<Fp31, MM, 8, 5, 4>(),
+    unit_entry<Fp31, MM, 4, 6, 1>(),
+    unit_entry<Fp31, MM, 10, 6, 8>(),
+    unit_entry<Fp31, MM, 6, 7, 2>(),
+    unit_entry<Fp31, MM, 9, 7, 4>(),
+    unit_entry<Fp31, MM, 5, 9, 1>(),
+    unit_entry<Fp31, MM, 8, 9, 4>(),
+    unit_entry<Fp31, MM, 4, 10, 1>(),
+    unit_entry<Fp31, MM, 8, 10, 4>(),
+)

@@ -3,20 +3,15 @@
 // the 64 KB of constant memory per module.
 #include "bg_inst_common.cuh"
 
-const SweepEntry* bg_entries_grid2(int* count)
-{
-    static const SweepEntry table[] = {
-        unit_entry<Fp31, 6, 5, 2>(BG_FIELD_FP31),
-        unit_entry<Fp31, 9, 5, 4>(BG_FIELD_FP31),
-        unit_entry<Fp31, 5, 6, 1>(BG_FIELD_FP31),
-        unit_entry<Fp31, 4, 7, 1>(BG_FIELD_FP31),
-        unit_entry<Fp31, 7, 7, 4>(BG_FIELD_FP31),
-        unit_entry<Fp31, 10, 7, 8>(BG_FIELD_FP31),
-        unit_entry<Fp31, 6, 9, 2>(BG_FIELD_FP31),
-        unit_entry<Fp31, 9, 9, 4>(BG_FIELD_FP31),
-        unit_entry<Fp31, 5, 10, 1>(BG_FIELD_FP31),
-        unit_entry<Fp31, 10, 10, 8>(BG_FIELD_FP31),
-    };
-    *count = (int)(sizeof(table) / sizeof(table[0]));
-    return table;
-}
+BG_DEFINE_TABLE(grid2,
+    unit_entry<Fp31, MM, 6, 5, 2>(),
+    unit_entry<Fp31, MM, 9, 5, 4>(),
+    unit_entry<Fp31, MM, 5, 6, 1>(),
+    unit_entry<Fp31, MM, 4, 7, 1>(),
+    unit_entry<Fp31, MM, 7, 7, 4>(),
+    unit_entry<Fp31, MM, 10, 7, 8>(),
+    unit_entry<Fp31, MM, 6, 9, 2>(),
+    unit_entry<Fp31, MM, 9, 9, 4>(),
+    unit_entry<Fp31, MM, 5, 10, 1>(),
+    unit_entry<Fp31, MM, 10, 10, 8>(),
+)

@@ -3,27 +3,21 @@
 // n = 9 up to d = 10, d = 8 for the leg scan), so that they do not fall to the general kernel.
 #include "bg_inst_common.cuh"
 
-const SweepEntry* bg_entries_paper(int* count)
-{
-    static const SweepEntry table[] = {
-        unit_entry<Fp31, 6, 4, 2>(BG_FIELD_FP31),
-        unit_entry<Fp31, 8, 4, 4>(BG_FIELD_FP31),
-        unit_entry<Fp31, 9, 4, 4>(BG_FIELD_FP31),
-        unit_entry<Fp31, 6, 6, 2>(BG_FIELD_FP31),
-        unit_entry<Fp31, 9, 6, 4>(BG_FIELD_FP31),
-        unit_entry<Fp31, 6, 8, 2>(BG_FIELD_FP31),
-        unit_entry<Fp31, 8, 8, 4>(BG_FIELD_FP31),
-        unit_entry<Fp31, 9, 8, 4>(BG_FIELD_FP31),
-        unit_entry<Fp31, 6, 10, 2>(BG_FIELD_FP31),
-        unit_entry<Fp31, 9, 10, 4>(BG_FIELD_FP31),
-        // the rest of the leg scans n = 4..10 at d = 4 and d = 8 (the configs cover (4,4), (10,8))
-        unit_entry<Fp31, 5, 4, 1>(BG_FIELD_FP31),
-        unit_entry<Fp31, 7, 4, 4>(BG_FIELD_FP31),
-        unit_entry<Fp31, 10, 4, 8>(BG_FIELD_FP31),
-        unit_entry<Fp31, 4, 8, 1>(BG_FIELD_FP31),
-        unit_entry<Fp31, 5, 8, 1>(BG_FIELD_FP31),
-        unit_entry<Fp31, 7, 8, 4>(BG_FIELD_FP31),
-    };
-    *count = (int)(sizeof(table) / sizeof(table[0]));
-    return table;
-}
+BG_DEFINE_TABLE(paper,
+    unit_entry<Fp31, MM, 6, 4, 2>(),
+    unit_entry<Fp31, MM, 8, 4, 4>(),
+    unit_entry<Fp31, MM, 9, 4, 4>(),
+    unit_entry<Fp31, MM, 6, 6, 2>(),
+    unit_entry<Fp31, MM, 9, 6, 4>(),
+    unit_entry<Fp31, MM, 6, 8, 2>(),
+    unit_entry<Fp31, MM, 8, 8, 4>(),
+    unit_entry<Fp31, MM, 9, 8, 4>(),
+    unit_entry<Fp31, MM, 6, 10, 2>(),
+    unit_entry<Fp31, MM, 9, 10, 4>(),
+    unit_entry<Fp31, MM, 5, 4, 1>(),
+    unit_entry<Fp31, MM, 7, 4, 4>(),
+    unit_entry<Fp31, MM, 10, 4, 8>(),
+    unit_entry<Fp31, MM, 4, 8, 1>(),
+    unit_entry<Fp31, MM, 5, 8, 1>(),
+    unit_entry<Fp31, MM, 7, 8, 4>(),
+)

@@ -15,14 +15,10 @@
 // of the two lanes' partial products (bg_split.cuh).  Inputs are read straight from global memory
 // into registers (32 contiguous bytes per lane and row).
 #pragma once
-#include "bg_field.cuh"
-#include "bg_recursion.cuh"
-#include "bg_tables.cuh"
-#include "bg_tile.cuh"
-#include "bg_split.cuh"
+#include "bg_common.cuh"
+#include "bg_schedule.cuh"
 
 namespace bg {
-
 template <class F, int N, int D>
 struct RegCfg {
     typedef typename F::E E;
@@ -43,8 +39,24 @@ struct RegCfg {
 template <int N>
 __host__ __device__ constexpr int reg_row(int i, int len) { return tt_row(N, i, len); }
 
-template <class F, int N, int D>
-__global__ void __launch_bounds__(32 * RegCfg<F, N, D>::WARPS, RegCfg<F, N, D>::MIN_BLOCKS) bg_reg_kernel(const TileParams<typename F::E> prm)
+// -(x.y) of two vectors held as (lane 0: components 0..DL-1, lane 1: the rest); full value in both lanes
+template <class F, int MET, int DL, int TP>
+__device__ __forceinline__ typename F::E reg_dot_neg(const F& f, int mu0, const typename F::E (&x)[DL],
+                                                     const typename F::E (&y)[DL])
+{
+    typename F::E nx[DL];
+    lower_neg<F, MET, DL>(f, mu0, x, nx);
+    return lane_sum<F, 2, TP>(f, f.reduce(dot_plain<F, DL>(f, nx, y)));
+}
+template <class F, int DL, int TP>
+__device__ __forceinline__ typename F::E reg_dot_plain(const F& f, const typename F::E (&x)[DL],
+                                                       const typename F::E (&y)[DL])
+{
+    return lane_sum<F, 2, TP>(f, f.reduce(dot_plain<F, DL>(f, x, y)));
+}
+
+template <class F, int MET, int N, int D>
+__global__ void __launch_bounds__(32 * RegCfg<F, N, D>::WARPS, RegCfg<F, N, D>::MIN_BLOCKS) bg_reg_kernel(const BgParams<F> prm)
 {
     typedef RegCfg<F, N, D> C;
     typedef typename F::E E;
@@ -52,8 +64,8 @@ __global__ void __launch_bounds__(32 * RegCfg<F, N, D>::WARPS, RegCfg<F, N, D>::
     constexpr int M = C::M, DL = C::DL, TP = C::TP, ND = N * D;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int point = lane & (TP - 1), half = lane / TP;
-    const bool t0 = half == 0;                                 // this lane owns the time component
+    const int point = lane & (TP - 1), half = lane / TP, mu0 = half * DL;
+    const F f(prm.fld, 0);
     E* sc = reinterpret_cast<E*>(smem_raw) + (size_t)warp * C::NSCAL * TP + point;   // [index][TP], this point's column
     const long long pt = ((long long)blockIdx.x * C::WARPS + warp) * TP + point;
     const bool live = pt < prm.batch;
@@ -69,23 +81,23 @@ __global__ void __launch_bounds__(32 * RegCfg<F, N, D>::WARPS, RegCfg<F, N, D>::
         E run[DL];
 #pragma unroll
         for (int mu = 0; mu < DL; ++mu) {
-            run[mu] = F::ezero();
+            run[mu] = f.ezero();
             sc[(C::PS_OFF + mu + half * DL) * TP] = run[mu];
         }
 #pragma unroll
         for (int c = 1; c <= N; ++c) {
 #pragma unroll
-            for (int mu = 0; mu < DL; ++mu) J[c - 1][mu] = F::load_input(__ldg(gp + (c - 1) * D + mu));
+            for (int mu = 0; mu < DL; ++mu) J[c - 1][mu] = f.load_input(__ldg(gp + (c - 1) * D + mu));
             if (c <= M) {
                 E k[DL];
 #pragma unroll
-                for (int mu = 0; mu < DL; ++mu) k[mu] = F::dbl(F::load_input(__ldg(gm + (c - 1) * D + mu)));
-                const E u = F::neg(split_dot_neg<F, DL, TP>(t0, k, J[c - 1]));       // 2 k.eps
+                for (int mu = 0; mu < DL; ++mu) k[mu] = f.dbl(f.load_input(__ldg(gm + (c - 1) * D + mu)));
+                const E u = f.neg(reg_dot_neg<F, MET, DL, TP>(f, mu0, k, J[c - 1]));       // 2 k.eps
                 sc[(C::U_OFF + c - 1) * TP] = u;
                 sc[(C::V_OFF + c - 1) * TP] = u;
 #pragma unroll
                 for (int mu = 0; mu < DL; ++mu) {
-                    run[mu] = F::add(run[mu], k[mu]);
+                    run[mu] = f.add(run[mu], k[mu]);
                     sc[(C::PS_OFF + c * D + mu + half * DL) * TP] = run[mu];
                 }
             }
@@ -103,18 +115,17 @@ __global__ void __launch_bounds__(32 * RegCfg<F, N, D>::WARPS, RegCfg<F, N, D>::
             for (int mu = 0; mu < DL; ++mu) {
                 l[mu] = sc[(C::PS_OFF + ci * D + mu + half * DL) * TP];            // PS2_{i-1}
                 h[mu] = sc[(C::PS_OFF + (ci + L) * D + mu + half * DL) * TP];      // PS2_j
-                x2[mu] = F::sub(l[mu], h[mu]);
             }
-            x2[0] = cneg(x2[0], t0);                                                 // 2 * covariant P_{i,j}
+            lower_diff<F, MET, DL>(f, mu0, h, l, x2);                                // 2 * covariant P_{i,j}
             A acc[DL];
 #pragma unroll
-            for (int mu = 0; mu < DL; ++mu) acc[mu] = F::zero();
-            E hsum = F::ezero();
+            for (int mu = 0; mu < DL; ++mu) acc[mu] = f.zero();
+            E hsum = f.ezero();
             int room = F::kCap0;
             auto need = [&](int k) {
                 if (room < k) {
 #pragma unroll
-                    for (int mu = 0; mu < DL; ++mu) acc[mu] = F::relief(acc[mu]);
+                    for (int mu = 0; mu < DL; ++mu) acc[mu] = f.relief(acc[mu]);
                     room = F::kCapR;
                 }
                 room -= k;
@@ -126,62 +137,62 @@ __global__ void __launch_bounds__(32 * RegCfg<F, N, D>::WARPS, RegCfg<F, N, D>::
 #pragma unroll
                 for (int mu = 0; mu < DL; ++mu) s[mu] = sc[(C::PS_OFF + (ci + la) * D + mu + half * DL) * TP];
                 const E ua = sc[(C::U_OFF + ra) * TP], vb = sc[(C::V_OFF + rb) * TP];
-                const E hk = F::neg(split_dot_neg<F, DL, TP>(t0, J[ra], J[rb]));    // A.B
-                const E xa = split_dot_plain<F, DL, TP>(x2, J[ra]);                 // 2 X.A
-                const E xb = split_dot_plain<F, DL, TP>(x2, J[rb]);                 // 2 X.B
-                const E cb = F::sub(xa, ua);
-                const E ca = F::sub(vb, xb);
-                hsum = F::add(hsum, hk);
+                const E hk = f.neg(reg_dot_neg<F, MET, DL, TP>(f, mu0, J[ra], J[rb]));    // A.B
+                const E xa = reg_dot_plain<F, DL, TP>(f, x2, J[ra]);                 // 2 X.A
+                const E xb = reg_dot_plain<F, DL, TP>(f, x2, J[rb]);                 // 2 X.B
+                const E cb = f.sub(xa, ua);
+                const E ca = f.sub(vb, xb);
+                hsum = f.add(hsum, hk);
                 need(2);
 #pragma unroll
                 for (int mu = 0; mu < DL; ++mu) {
-                    acc[mu] = F::mad(hk, s[mu], acc[mu]);
-                    acc[mu] = F::mad(cb, J[rb][mu], acc[mu]);
+                    acc[mu] = f.mad(hk, s[mu], acc[mu]);
+                    acc[mu] = f.mad(cb, J[rb][mu], acc[mu]);
                 }
                 need(1);
 #pragma unroll
-                for (int mu = 0; mu < DL; ++mu) acc[mu] = F::mad(ca, J[ra][mu], acc[mu]);
+                for (int mu = 0; mu < DL; ++mu) acc[mu] = f.mad(ca, J[ra][mu], acc[mu]);
 #pragma unroll
                 for (int lb = 1; lb <= L - la - 1; ++lb) {
                     const int rm = reg_row<N>(i + la, lb), rc = reg_row<N>(i + la + lb, L - la - lb);
-                    const E cc = F::neg(F::dbl(split_dot_neg<F, DL, TP>(t0, J[ra], J[rc])));   // 2 A.C
+                    const E cc = f.neg(f.dbl(reg_dot_neg<F, MET, DL, TP>(f, mu0, J[ra], J[rc])));   // 2 A.C
                     need(1);
 #pragma unroll
-                    for (int mu = 0; mu < DL; ++mu) acc[mu] = F::mad(cc, J[rm][mu], acc[mu]);
+                    for (int mu = 0; mu < DL; ++mu) acc[mu] = f.mad(cc, J[rm][mu], acc[mu]);
                 }
             }
             // ---- finish: boundary term of the (P-Q) sum, propagator, U and V --------------------------
-            const E nhh = F::neg(F::mul(hsum, F::half()));                          // -(sum_k h_k)/2
+            const E nhh = f.neg(f.mul(hsum, f.half()));                          // -(sum_k h_k)/2
             need(2);
 #pragma unroll
             for (int mu = 0; mu < DL; ++mu) {
-                acc[mu] = F::mad(nhh, l[mu], acc[mu]);
-                acc[mu] = F::mad(nhh, h[mu], acc[mu]);
+                acc[mu] = f.mad(nhh, l[mu], acc[mu]);
+                acc[mu] = f.mad(nhh, h[mu], acc[mu]);
             }
             const int own = L < M ? reg_row<N>(i, L) : C::J_ROWS;
             if (L < M) {
                 E xc[DL];
 #pragma unroll
-                for (int mu = 0; mu < DL; ++mu) xc[mu] = F::sub(h[mu], l[mu]);      // 2 P_{i,j}, contravariant
-                const E s4 = F::canon(F::neg(split_dot_neg<F, DL, TP>(t0, xc, xc)));  // 4 P^2
-                if (F::is_zero(s4)) status |= 1u;
-                const E w = F::dbl(F::dbl(F::inv(s4)));                              // 1/P^2, inv(0) := 0
+                for (int mu = 0; mu < DL; ++mu) xc[mu] = f.sub(h[mu], l[mu]);      // 2 P_{i,j}, contravariant
+                const E s4 = f.canon(f.neg(reg_dot_neg<F, MET, DL, TP>(f, mu0, xc, xc)));  // 4 P^2
+                if (f.is_zero(s4)) status |= 1u;
+                const E w = f.dbl(f.dbl(f.inv(s4)));                              // 1/P^2, inv(0) := 0
 #pragma unroll
-                for (int mu = 0; mu < DL; ++mu) J[own][mu] = F::mul(F::reduce(acc[mu]), w);
-                const E c2 = split_dot_plain<F, DL, TP>(x2, J[own]);                 // 2 P_{i,j} . J(i..j)
-                sc[(C::U_OFF + own) * TP] = F::add(c2, hsum);
-                sc[(C::V_OFF + own) * TP] = F::sub(c2, hsum);
+                for (int mu = 0; mu < DL; ++mu) J[own][mu] = f.mul(f.reduce(acc[mu]), w);
+                const E c2 = reg_dot_plain<F, DL, TP>(f, x2, J[own]);                 // 2 P_{i,j} . J(i..j)
+                sc[(C::U_OFF + own) * TP] = f.add(c2, hsum);
+                sc[(C::V_OFF + own) * TP] = f.sub(c2, hsum);
             } else {
                 // top current: no propagator; amplitude = eps_n . N(1..m)
 #pragma unroll
-                for (int mu = 0; mu < DL; ++mu) J[own][mu] = F::reduce(acc[mu]);
-                const E nout = split_dot_neg<F, DL, TP>(t0, J[N - 1], J[own]);
-                if (live && half == 0) prm.out[pt] = F::canon(F::neg(nout));
+                for (int mu = 0; mu < DL; ++mu) J[own][mu] = f.reduce(acc[mu]);
+                const E nout = reg_dot_neg<F, MET, DL, TP>(f, mu0, J[N - 1], J[own]);
+                if (live && half == 0) prm.out[pt] = f.to_output(f.neg(nout));
             }
             if (prm.currents && live) {
                 E* dst = prm.currents + (pt * M * M + (long long)ci * M + (ci + L - 1)) * D + half * DL;
 #pragma unroll
-                for (int mu = 0; mu < DL; ++mu) dst[mu] = F::canon(J[own][mu]);
+                for (int mu = 0; mu < DL; ++mu) dst[mu] = f.to_output(J[own][mu]);
             }
         }
     }
@@ -190,7 +201,7 @@ __global__ void __launch_bounds__(32 * RegCfg<F, N, D>::WARPS, RegCfg<F, N, D>::
         for (int c = 0; c < M; ++c) {
             E* dst = prm.currents + (pt * M * M + (long long)c * M + c) * D + half * DL;
 #pragma unroll
-            for (int mu = 0; mu < DL; ++mu) dst[mu] = F::canon(J[c][mu]);
+            for (int mu = 0; mu < DL; ++mu) dst[mu] = f.to_output(J[c][mu]);
         }
     }
     if (prm.status && live && half == 0) prm.status[pt] = status;

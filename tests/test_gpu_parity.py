@@ -29,6 +29,15 @@ def bgl():
     return binding
 
 
+@pytest.fixture
+def select_kernel(bgl):
+    """restrict the kernel selection for one test (bg_set_kernel_override), default again afterwards"""
+    def choose(kind, warps=0):
+        bgl.bg_set_kernel_override(kind, warps)
+    yield choose
+    bgl.bg_set_kernel_override("default", 0)
+
+
 def _gpu_amplitudes(bgl, mom, pol, want_status=False):
     import torch
     dm, dp = bgl.to_device(mom), bgl.to_device(pol)
@@ -170,7 +179,8 @@ def test_error_codes(bgl):
     assert bgl.bg_amplitudes(0, 3, 4, 8, p, p + 1024, p + 2048, 0) == bgl.BG_ERR_ARG      # n too small
     assert bgl.bg_amplitudes(0, 17, 4, 8, p, p + 1024, p + 2048, 0) == bgl.BG_ERR_ARG
     assert bgl.bg_amplitudes(0, 4, 3, 8, p, p + 1024, p + 2048, 0) == bgl.BG_ERR_ARG      # d too small
-    assert bgl.bg_amplitudes(2, 4, 4, 8, p, p + 1024, p + 2048, 0) == bgl.BG_ERR_ARG      # field
+    assert bgl.bg_amplitudes(3, 4, 4, 8, p, p + 1024, p + 2048, 0) == bgl.BG_ERR_ARG      # field
+    assert bgl.bg_amplitudes(2, 4, 4, 8, p, p + 1024, p + 2048, 0) == bgl.BG_ERR_ARG      # FPMONT needs a prime
     assert bgl.bg_amplitudes(0, 4, 4, -1, p, p + 1024, p + 2048, 0) == bgl.BG_ERR_ARG     # batch
     assert bgl.bg_amplitudes(0, 4, 4, 8, 0, p + 1024, p + 2048, 0) == bgl.BG_ERR_ARG      # null
     assert bgl.bg_amplitudes(0, 4, 4, 8, p + 4, p + 1024, p + 2048, 0) == bgl.BG_ERR_ARG  # misaligned
@@ -226,29 +236,27 @@ def test_full_size_complex(bgl, oracle_mod, name):
         assert np.median(rel) < 1e-12 and np.mean(rel < 1e-9) > 0.995
 
 
-# ---- every compiled kernel family / warps-per-tile variant (selection knobs BG_KERNEL, BG_SWEEP_W) ---
-VARIANTS = [("fp31", 8, 6, "level", 4), ("fp31", 8, 6, "level", 6), ("fp31", 8, 6, "tile", 4),
-            ("fp31", 4, 4, "level", 1), ("fp31", 4, 4, "tile", 1),
-            ("fp31", 10, 8, "tile", 8), ("fp31", 12, 6, "tile", 16),
-            ("c128", 6, 4, "level", 2), ("c128", 6, 4, "level", 4), ("c128", 6, 4, "tile", 4),
-            ("c128", 6, 4, "tile", 2), ("fp31", 8, 6, "general", 0), ("c128", 6, 4, "general", 0),
-            ("c128", 12, 6, "split", 16), ("c128", 6, 4, "split", 2), ("c128", 6, 4, "split", 4),
-            ("c128", 6, 4, "reg", 4), ("fp31", 8, 6, "unit", 4),
-            ("fp31", 10, 8, "unit", 8), ("fp31", 12, 6, "unit", 8),
+# ---- every compiled kernel family / warps-per-tile variant (bg_set_kernel_override) --------------------
+VARIANTS = [("fp31", 8, 6, "unit1", 4), ("fp31", 8, 6, "unit1", 6), ("fp31", 8, 6, "unit1", 2),
+            ("fp31", 4, 4, "unit1", 1), ("fp31", 10, 8, "unit1", 8), ("fp31", 10, 8, "unit1", 4),
+            ("fp31", 12, 6, "unit1", 8), ("fp31", 12, 6, "unit1", 16), ("fp31", 12, 6, "unit1", 4),
+            ("fp31", 8, 6, "general", 0), ("fp31", 12, 6, "general", 0), ("c128", 6, 4, "general", 0),
+            ("c128", 6, 4, "reg", 4), ("c128", 6, 4, "unit2", 2), ("c128", 6, 4, "unit2", 4),
+            ("c128", 6, 4, "unit1", 2), ("c128", 6, 4, "unit1", 4),
+            ("c128", 12, 6, "unit2", 16), ("c128", 12, 6, "unit2", 8),
             # the shapes of the paper's own benchmarks (bg_inst_paper.cu)
-            ("fp31", 6, 4, "unit", 2), ("fp31", 8, 4, "unit", 4), ("fp31", 9, 4, "unit", 4), ("fp31", 6, 6, "unit", 2),
-            ("fp31", 9, 6, "unit", 4), ("fp31", 6, 8, "unit", 2), ("fp31", 8, 8, "unit", 4), ("fp31", 9, 8, "unit", 4),
-            ("fp31", 6, 10, "unit", 2), ("fp31", 9, 10, "unit", 4), ("fp31", 5, 4, "unit", 1), ("fp31", 7, 4, "unit", 4),
-            ("fp31", 10, 4, "unit", 8), ("fp31", 4, 8, "unit", 1), ("fp31", 5, 8, "unit", 1), ("fp31", 7, 8, "unit", 4)]
+            ("fp31", 6, 4, "unit1", 2), ("fp31", 8, 4, "unit1", 4), ("fp31", 9, 4, "unit1", 4), ("fp31", 6, 6, "unit1", 2),
+            ("fp31", 9, 6, "unit1", 4), ("fp31", 6, 8, "unit1", 2), ("fp31", 8, 8, "unit1", 4), ("fp31", 9, 8, "unit1", 4),
+            ("fp31", 6, 10, "unit1", 2), ("fp31", 9, 10, "unit1", 4), ("fp31", 5, 4, "unit1", 1), ("fp31", 7, 4, "unit1", 4),
+            ("fp31", 10, 4, "unit1", 8), ("fp31", 4, 8, "unit1", 1), ("fp31", 5, 8, "unit1", 1), ("fp31", 7, 8, "unit1", 4)]
+KIND_ID = {"general": 0, "unit1": 1, "unit2": 2, "reg": 3}
 
 
 @pytest.mark.parametrize("field,n,d,kernel,w", VARIANTS, ids=lambda v: str(v))
-def test_kernel_variants(bgl, oracle_mod, monkeypatch, field, n, d, kernel, w):
-    if kernel == "general":
-        monkeypatch.setenv("BG_SWEEP_W", "0")               # the runtime-n kernel
-    else:
-        monkeypatch.setenv("BG_KERNEL", kernel)
-        monkeypatch.setenv("BG_SWEEP_W", str(w))
+def test_kernel_variants(bgl, oracle_mod, select_kernel, field, n, d, kernel, w):
+    select_kernel(kernel, w)
+    ki = bgl.bg_kernel_info(bgl.FIELD_FP31 if field == "fp31" else bgl.FIELD_C128, n, d)
+    assert ki["specialised"] == KIND_ID[kernel] and (kernel == "general" or ki["threads_per_block"] == 32 * w)
     batch = 203                                              # six full tiles and a ragged one
     if field == "fp31":
         mom, pol, _ = inputs.make_fp_inputs(n, d, batch, seed=31)
@@ -319,20 +327,17 @@ def _extreme_inputs(kind, n, d, batch):
 
 
 EXTREME_KINDS = ["all_p-1", "raw_2p_and_2p+1", "p-1_alternating_1", "mixed", "4d_zero_padded"]
-EXTREME_CASES = [(8, 6, "level", 4), (8, 6, "level", 6), (8, 6, "tile", 4), (8, 6, "unit", 4), (8, 6, "general", 0),
-                 (12, 6, "unit", 8), (12, 6, "tile", 16), (12, 6, "general", 0),
-                 (10, 8, "unit", 8), (10, 8, "tile", 8), (10, 8, "general", 0),
-                 (4, 4, "level", 1), (4, 4, "tile", 1), (9, 10, "unit", 4),
+EXTREME_CASES = [(8, 6, "unit1", 4), (8, 6, "unit1", 6), (8, 6, "unit1", 2), (8, 6, "general", 0),
+                 (12, 6, "unit1", 8), (12, 6, "unit1", 16), (12, 6, "general", 0),
+                 (10, 8, "unit1", 8), (10, 8, "unit1", 4), (10, 8, "general", 0),
+                 (4, 4, "unit1", 1), (4, 4, "general", 0), (9, 10, "unit1", 4), (7, 5, "unit1", 4),
                  (5, 16, "general", 0), (16, 4, "general", 0), (16, 16, "general", 0)]
 
 
 @pytest.mark.parametrize("n,d,kernel,w", EXTREME_CASES, ids=lambda v: str(v))
-def test_fp_extreme_residues(bgl, oracle_mod, monkeypatch, n, d, kernel, w):
-    if kernel == "general":
-        monkeypatch.setenv("BG_SWEEP_W", "0")
-    else:
-        monkeypatch.setenv("BG_KERNEL", kernel)
-        monkeypatch.setenv("BG_SWEEP_W", str(w))
+def test_fp_extreme_residues(bgl, oracle_mod, select_kernel, n, d, kernel, w):
+    select_kernel(kernel, w)
+    assert bgl.bg_kernel_info(bgl.FIELD_FP31, n, d)["specialised"] == KIND_ID[kernel]
     batch = 70
     iu = np.triu_indices(n - 1)
     for kind in EXTREME_KINDS:
