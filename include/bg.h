@@ -68,6 +68,7 @@ typedef struct CUstream_st* cudaStream_t;
 typedef enum { BG_FIELD_FP31 = 0, BG_FIELD_C128 = 1, BG_FIELD_FPMONT = 2 } bg_field_t;
 typedef enum { BG_METRIC_MOSTLY_MINUS = 0, BG_METRIC_ALTERNATING = 1 } bg_metric_t;
 #define BG_MAX_PRIMES 8
+#define BG_MAX_TREES 8
 
 typedef enum {
     BG_OK = 0,
@@ -131,6 +132,14 @@ int bg_amplitudes_states(int field, int n, int d, int64_t batch, int states, con
 int bg_amplitudes_primes(int metric, int n, int d, int64_t batch, int n_primes, const uint32_t* primes,
                          const void* momenta, const void* polarisations, void* out, uint32_t* status,
                          cudaStream_t stream);
+
+/* The left-hand side of the cut equation Eq.(4), PAPER.md:79-81 -- "sum over states" of the product of
+ * the tree amplitudes of a cut:  out[b] = sum_{s<S} prod_{t<trees} amps[t][b][s].
+ * amps: HOST array of `trees` (1..BG_MAX_TREES) DEVICE pointers, each [batch][S] scalars as written by
+ * bg_amplitudes_states / bg_evaluate; out: device [batch], must not alias an input.  prime: the
+ * modulus for BG_FIELD_FPMONT (plain residues in and out), ignored otherwise. */
+int bg_state_sum(int field, uint32_t prime, int64_t batch, int states, int trees,
+                 const void* const* amps, void* out, cudaStream_t stream);
 
 /* End-to-end variant with HOST buffers (pinned memory recommended): copies the inputs to
  * the device in chunks, runs the kernel and copies the results back, overlapping the three

@@ -26,7 +26,7 @@ PEAK_KINDS = {"imad_wide": 0, "imad": 1, "alu": 2, "mix": 3, "modmul": 4, "dfma"
 P31 = (1 << 31) - 1
 
 EXPORTS = ["bg_amplitudes", "bg_amplitudes_status", "bg_currents", "bg_evaluate", "bg_amplitudes_states",
-           "bg_amplitudes_primes", "bg_amplitudes_host", "bg_host_workspace_bytes", "bg_modulus",
+           "bg_amplitudes_primes", "bg_state_sum", "bg_amplitudes_host", "bg_host_workspace_bytes", "bg_modulus",
            "bg_status_string", "bg_version", "bg_op_count", "bg_kernel_info", "bg_kernel_info_problem",
            "bg_set_kernel_override", "bg_peak_probe", "bg_selftest_schedules"]
 
@@ -85,6 +85,8 @@ def load(rebuild_if_stale: bool = False):
     lib.bg_evaluate.argtypes = [ctypes.POINTER(Problem), i64, vp, vp, vp, vp, vp, vp]
     lib.bg_amplitudes_states.argtypes = [ci, ci, ci, i64, ci, vp, vp, vp, vp, vp]
     lib.bg_amplitudes_primes.argtypes = [ci, ci, ci, i64, ci, ctypes.POINTER(ctypes.c_uint32), vp, vp, vp, vp, vp]
+    lib.bg_state_sum.argtypes = [ci, ctypes.c_uint32, i64, ci, ci, ctypes.POINTER(vp), vp, vp]
+    lib.bg_state_sum.restype = ci
     lib.bg_kernel_info_problem.argtypes = [ctypes.POINTER(Problem), ctypes.POINTER(KernelInfo)]
     lib.bg_set_kernel_override.argtypes = [ci, ci]
     lib.bg_amplitudes_host.argtypes = [ci, ci, ci, i64, vp, vp, vp, vp, vp, sz]
@@ -144,6 +146,11 @@ def bg_amplitudes_primes(metric, n, d, batch, primes, momenta_ptr, polarisations
     arr = (ctypes.c_uint32 * len(primes))(*primes)
     return load().bg_amplitudes_primes(metric, n, d, batch, len(primes), arr, momenta_ptr, polarisations_ptr,
                                        out_ptr, status_ptr, stream_ptr)
+
+
+def bg_state_sum(field, prime, batch, states, amp_ptrs, out_ptr, stream_ptr=0):
+    arr = (ctypes.c_void_p * len(amp_ptrs))(*amp_ptrs)
+    return load().bg_state_sum(field, prime, batch, states, len(amp_ptrs), arr, out_ptr, stream_ptr)
 
 
 def bg_set_kernel_override(kind=-1, warps=0):
@@ -283,6 +290,21 @@ def evaluate(momenta, polarisations, metric=METRIC_MOSTLY_MINUS, primes=(), stat
     with torch.cuda.device(momenta.device):
         _check(bg_evaluate(pb, batch, momenta.data_ptr(), polarisations.data_ptr(), out.data_ptr(), None,
                            None if status is None else status.data_ptr(), s))
+    return out
+
+
+def state_sum(amps, prime=0, stream=None):
+    """out[b] = sum_s prod_t amps[t][b, s] (Eq.(4)) for a list of [batch, S] CUDA tensors"""
+    torch = _torch()
+    a0 = amps[0]
+    if any(a.shape != a0.shape or a.dtype != a0.dtype or not a.is_cuda or not a.is_contiguous() for a in amps) \
+            or a0.dim() != 2:
+        raise BgError("amps must be contiguous CUDA tensors [batch, S] of one dtype")
+    field = FIELD_FPMONT if prime else field_of(a0)
+    out = torch.empty(a0.shape[0], dtype=a0.dtype, device=a0.device)
+    s = (stream or torch.cuda.current_stream(a0.device)).cuda_stream
+    with torch.cuda.device(a0.device):
+        _check(bg_state_sum(field, prime, a0.shape[0], a0.shape[1], [a.data_ptr() for a in amps], out.data_ptr(), s))
     return out
 
 

@@ -191,8 +191,10 @@ int ensure_attr(Launch* L)
     return BG_OK;
 }
 
-// ---- Montgomery constants of a prime ------------------------------------------------------------------
-bool mont_constants(uint32_t p, int i, FpMont::Params* q)
+}  // namespace
+
+// ---- Montgomery constants of a prime (also used by bg_state_sum.cu) ----------------------------------
+bool bg_mont_constants(uint32_t p, int i, bg::FpMont::Params* q)
 {
     if (!(p & 1u) || p <= (1u << 30) || p >= (1u << 31)) return false;
     uint32_t inv = p;                                  // Newton: inv = p^-1 mod 2^32 (p odd; 3 bits correct at start)
@@ -205,6 +207,8 @@ bool mont_constants(uint32_t p, int i, FpMont::Params* q)
     q->half[i] = (uint32_t)(r * ((p + 1u) / 2u) % p);
     return true;
 }
+
+namespace {
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
@@ -259,7 +263,7 @@ int run(const bg_problem_t& pb, int64_t batch, const void* mom, const void* pol,
     FpMont::Params mont{};
     if (pb.field == BG_FIELD_FPMONT)
         for (int i = 0; i < pb.n_primes; ++i)
-            if (!mont_constants(pb.primes[i], i, &mont)) return BG_ERR_ARG;
+            if (!bg_mont_constants(pb.primes[i], i, &mont)) return BG_ERR_ARG;
     Launch* L = nullptr;
     rc = select(pb.field, pb.metric, pb.n, pb.d, pb.states > 1, &L);
     if (rc != BG_OK) return rc;

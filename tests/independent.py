@@ -21,55 +21,104 @@ P31 = (1 << 31) - 1
 
 
 class Fp:
+    """exact arithmetic mod P with Python ints; subclasses made by fp_class(p) use another prime"""
     __slots__ = ("v",)
+    P = P31
 
     def __init__(self, v):
-        self.v = int(v) % P31
+        self.v = int(v) % self.P
 
     def __add__(self, o):
-        return Fp(self.v + _v(o))
+        return type(self)(self.v + _v(o))
 
     __radd__ = __add__
 
     def __sub__(self, o):
-        return Fp(self.v - _v(o))
+        return type(self)(self.v - _v(o))
 
     def __rsub__(self, o):
-        return Fp(_v(o) - self.v)
+        return type(self)(_v(o) - self.v)
 
     def __mul__(self, o):
-        return Fp(self.v * _v(o))
+        return type(self)(self.v * _v(o))
 
     __rmul__ = __mul__
 
     def __neg__(self):
-        return Fp(-self.v)
+        return type(self)(-self.v)
 
     def __truediv__(self, o):
-        return Fp(self.v * pow(_v(o), P31 - 2, P31))
+        return type(self)(self.v * pow(_v(o), self.P - 2, self.P))
 
     def __rtruediv__(self, o):
-        return Fp(_v(o) * pow(self.v, P31 - 2, P31))
+        return type(self)(_v(o) * pow(self.v, self.P - 2, self.P))
 
     def __eq__(self, o):
-        return self.v == _v(o) % P31
+        return self.v == _v(o) % self.P
 
     def __repr__(self):
-        return f"Fp({self.v})"
+        return f"Fp({self.v} mod {self.P})"
+
+
+def fp_class(p: int):
+    """the same exact arithmetic modulo another prime (generic 31-bit primes)"""
+    return type(f"Fp_{p}", (Fp,), {"P": p, "__slots__": ()})
 
 
 def _v(o):
     return o.v if isinstance(o, Fp) else int(o)
 
 
-def frac_to_fp(x: Fraction) -> int:
-    return x.numerator % P31 * pow(x.denominator % P31, P31 - 2, P31) % P31
+def is_prime(n: int) -> bool:
+    """deterministic Miller-Rabin for n < 3.3e24 (first 13 primes as bases)"""
+    if n < 2:
+        return False
+    small = (2, 3, 5, 7, 11, 13, 17, 19, 23, 29, 31, 37, 41)
+    for q in small:
+        if n % q == 0:
+            return n == q
+    dd, r = n - 1, 0
+    while dd % 2 == 0:
+        dd //= 2
+        r += 1
+    for a in small:
+        x = pow(a, dd, n)
+        if x in (1, n - 1):
+            continue
+        for _ in range(r - 1):
+            x = x * x % n
+            if x == n - 1:
+                break
+        else:
+            return False
+    return True
+
+
+def frac_to_fp(x: Fraction, p: int = P31) -> int:
+    return x.numerator % p * pow(x.denominator % p, p - 2, p) % p
+
+
+_ALTERNATING = False
+
+
+class alternating_metric:
+    """context manager: every product below uses diag(+,-,+,-,...) instead of the
+    mostly-minus metric"""
+
+    def __enter__(self):
+        global _ALTERNATING
+        self.prev, _ALTERNATING = _ALTERNATING, True
+
+    def __exit__(self, *exc):
+        global _ALTERNATING
+        _ALTERNATING = self.prev
 
 
 def mdot(x, y):
     s = x[0] * y[0]
-    for a, b in zip(x[1:], y[1:]):
-        s = s - a * b
+    for mu in range(1, len(x)):
+        minus = (mu % 2 == 1) if _ALTERNATING else True
+        s = s - x[mu] * y[mu] if minus else s + x[mu] * y[mu]
     return s
 
 
