@@ -141,6 +141,29 @@ int bg_amplitudes_primes(int metric, int n, int d, int64_t batch, int n_primes, 
 int bg_state_sum(int field, uint32_t prime, int64_t batch, int states, int trees,
                  const void* const* amps, void* out, cudaStream_t stream);
 
+/* ---- the stage in front of the path, on the device ---------------------------- */
+
+/* The D-2 square-root-free polarisation states eps_x and their duals eps~_x (Eqs.(8)-(18))
+ * of `count` massless d-vectors: momenta [count][d], chi [count][4] (the massless 4-dimensional reference
+ * vector of Eq.(8)), eps and eps_tilde [count][d-2][d] (row x-1 = eps_x; eps~_1 = eps_2, eps~_2 = eps_1),
+ * status NULL or [count] (bit0: a denominator of Eqs.(10),(16)-(18) vanished, the states are undefined).
+ * 4 <= d <= 16.  prime: BG_FIELD_FPMONT only.  The mostly-minus spinors contain sqrt(-1): over F_p they
+ * exist only for p = 1 mod 4 (BG_ERR_UNSUPPORTED otherwise, in particular for BG_FIELD_FP31); with
+ * BG_METRIC_ALTERNATING they are rational.  Readings R13-R15 of DESIGN.md. */
+int bg_states(int field, uint32_t prime, int metric, int d, int64_t count, const void* momenta, const void* chi,
+              void* eps, void* eps_tilde, uint32_t* status, cudaStream_t stream);
+
+/* The seeded synthetic phase-space generator of DESIGN.md §4 (the recipe of BASELINE.json:configs; the
+ * paper draws its points on the host with lips) for points [start, start + batch) of the
+ * workload `seed`: momenta, polarisations (and references, NULL or the massless reference vectors r_i)
+ * [batch][n][d].  helicities: NULL for the generic transverse polarisations, else n signs (d = 4) for the
+ * spinor-helicity states on (k_i, r_i); redraws: NULL or one device counter, incremented by the number
+ * of rejected attempts (F_p).  Over F_p the result is bit-identical to the host generator
+ * (paper_2502_07060_b200/inputs.py), over complex128 it agrees to rounding. */
+int bg_generate(int field, uint32_t prime, int metric, int n, int d, int64_t batch, uint64_t seed, int64_t start,
+                const signed char* helicities, void* momenta, void* polarisations, void* references,
+                unsigned long long* redraws, cudaStream_t stream);
+
 /* End-to-end variant with HOST buffers (pinned memory recommended): copies the inputs to
  * the device in chunks, runs the kernel and copies the results back, overlapping the three
  * on internal streams; returns after everything has completed.  `workspace` is DEVICE

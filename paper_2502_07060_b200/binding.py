@@ -26,7 +26,7 @@ PEAK_KINDS = {"imad_wide": 0, "imad": 1, "alu": 2, "mix": 3, "modmul": 4, "dfma"
 P31 = (1 << 31) - 1
 
 EXPORTS = ["bg_amplitudes", "bg_amplitudes_status", "bg_currents", "bg_evaluate", "bg_amplitudes_states",
-           "bg_amplitudes_primes", "bg_state_sum", "bg_amplitudes_host", "bg_host_workspace_bytes", "bg_modulus",
+           "bg_amplitudes_primes", "bg_state_sum", "bg_states", "bg_generate", "bg_amplitudes_host", "bg_host_workspace_bytes", "bg_modulus",
            "bg_status_string", "bg_version", "bg_op_count", "bg_kernel_info", "bg_kernel_info_problem",
            "bg_set_kernel_override", "bg_peak_probe", "bg_selftest_schedules"]
 
@@ -87,6 +87,11 @@ def load(rebuild_if_stale: bool = False):
     lib.bg_amplitudes_primes.argtypes = [ci, ci, ci, i64, ci, ctypes.POINTER(ctypes.c_uint32), vp, vp, vp, vp, vp]
     lib.bg_state_sum.argtypes = [ci, ctypes.c_uint32, i64, ci, ci, ctypes.POINTER(vp), vp, vp]
     lib.bg_state_sum.restype = ci
+    lib.bg_states.argtypes = [ci, ctypes.c_uint32, ci, ci, i64, vp, vp, vp, vp, vp, vp]
+    lib.bg_states.restype = ci
+    lib.bg_generate.argtypes = [ci, ctypes.c_uint32, ci, ci, ci, i64, ctypes.c_uint64, i64, ctypes.c_char_p, vp, vp, vp,
+                                vp, vp]
+    lib.bg_generate.restype = ci
     lib.bg_kernel_info_problem.argtypes = [ctypes.POINTER(Problem), ctypes.POINTER(KernelInfo)]
     lib.bg_set_kernel_override.argtypes = [ci, ci]
     lib.bg_amplitudes_host.argtypes = [ci, ci, ci, i64, vp, vp, vp, vp, vp, sz]
@@ -151,6 +156,19 @@ def bg_amplitudes_primes(metric, n, d, batch, primes, momenta_ptr, polarisations
 def bg_state_sum(field, prime, batch, states, amp_ptrs, out_ptr, stream_ptr=0):
     arr = (ctypes.c_void_p * len(amp_ptrs))(*amp_ptrs)
     return load().bg_state_sum(field, prime, batch, states, len(amp_ptrs), arr, out_ptr, stream_ptr)
+
+
+def bg_states(field, prime, metric, d, count, momenta_ptr, chi_ptr, eps_ptr, eps_tilde_ptr, status_ptr=None,
+              stream_ptr=0):
+    return load().bg_states(field, prime, metric, d, count, momenta_ptr, chi_ptr, eps_ptr, eps_tilde_ptr, status_ptr,
+                            stream_ptr)
+
+
+def bg_generate(field, prime, metric, n, d, batch, seed, start, helicities, momenta_ptr, polarisations_ptr,
+                references_ptr=None, redraws_ptr=None, stream_ptr=0):
+    hel = None if helicities is None else bytes((int(h) & 0xFF) for h in helicities)
+    return load().bg_generate(field, prime, metric, n, d, batch, seed, start, hel, momenta_ptr, polarisations_ptr,
+                              references_ptr, redraws_ptr, stream_ptr)
 
 
 def bg_set_kernel_override(kind=-1, warps=0):
@@ -306,6 +324,40 @@ def state_sum(amps, prime=0, stream=None):
     with torch.cuda.device(a0.device):
         _check(bg_state_sum(field, prime, a0.shape[0], a0.shape[1], [a.data_ptr() for a in amps], out.data_ptr(), s))
     return out
+
+
+def _dtype_of(field):
+    import torch
+    return torch.complex128 if field == FIELD_C128 else torch.int32
+
+
+def generate(field, n, d, batch, seed=0, start=0, metric=METRIC_MOSTLY_MINUS, prime=0, helicities=None,
+             want_references=False, stream=None):
+    """seeded kinematics generated on the device (bg_generate): (momenta, polarisations[, references], redraws)"""
+    torch = _torch()
+    dt = _dtype_of(field)
+    mom = torch.empty((batch, n, d), dtype=dt, device="cuda")
+    pol = torch.empty((batch, n, d), dtype=dt, device="cuda")
+    ref = torch.empty((batch, n, d), dtype=dt, device="cuda") if want_references else None
+    redraws = torch.zeros(1, dtype=torch.int64, device="cuda")
+    s = (stream or torch.cuda.current_stream()).cuda_stream
+    _check(bg_generate(field, prime, metric, n, d, batch, seed, start, helicities, mom.data_ptr(), pol.data_ptr(),
+                       None if ref is None else ref.data_ptr(), redraws.data_ptr(), s))
+    return (mom, pol, ref, redraws) if want_references else (mom, pol, redraws)
+
+
+def states(momenta, chi, metric=METRIC_MOSTLY_MINUS, prime=0, stream=None):
+    """eps, eps_tilde [count, d-2, d] and status [count] for momenta [count, d], chi [count, 4] (bg_states)"""
+    torch = _torch()
+    count, d = momenta.shape
+    field = FIELD_FPMONT if prime else field_of(momenta)
+    eps = torch.empty((count, d - 2, d), dtype=momenta.dtype, device=momenta.device)
+    til = torch.empty_like(eps)
+    status = torch.zeros(count, dtype=torch.int32, device=momenta.device)
+    s = (stream or torch.cuda.current_stream(momenta.device)).cuda_stream
+    _check(bg_states(field, prime, metric, d, count, momenta.data_ptr(), chi.data_ptr(), eps.data_ptr(),
+                     til.data_ptr(), status.data_ptr(), s))
+    return eps, til, status
 
 
 def currents(momenta, polarisations, stream=None):

@@ -12,6 +12,7 @@
 #include "bg_common.cuh"
 #include "bg_entries.h"
 #include "bg_general.cuh"     // GeneralLayout (host side of the record layout)
+#include "bg_host_util.h"
 
 namespace {
 
@@ -205,6 +206,41 @@ bool bg_mont_constants(uint32_t p, int i, bg::FpMont::Params* q)
     q->one[i] = (uint32_t)r;
     q->r2[i] = (uint32_t)(r * r % p);
     q->half[i] = (uint32_t)(r * ((p + 1u) / 2u) % p);
+    return true;
+}
+
+namespace {
+
+uint64_t powmod(uint64_t a, uint64_t e, uint64_t p)
+{
+    uint64_t r = 1;
+    for (a %= p; e; e >>= 1) {
+        if (e & 1) r = r * a % p;
+        a = a * a % p;
+    }
+    return r;
+}
+
+}  // namespace
+
+bool bg_spinor_consts_fp(uint32_t p, int metric, const bg::FpMont::Params* q, uint32_t* jm, uint32_t* jv)
+{
+    uint64_t m, v;
+    if (metric == BG_METRIC_ALTERNATING) {
+        m = p - 1u;
+        v = 1u;
+    } else {
+        if (p % 4u != 1u) return false;
+        uint64_t g = 2;                                   // a quadratic non-residue: g^((p-1)/2) = -1
+        while (powmod(g, (p - 1u) / 2u, p) != p - 1u) ++g;
+        m = v = powmod(g, (p - 1u) / 4u, p);              // sqrt(-1)
+    }
+    if (q) {                                              // to Montgomery form: x R mod p
+        m = m * q->one[0] % p;
+        v = v * q->one[0] % p;
+    }
+    *jm = (uint32_t)m;
+    *jv = (uint32_t)v;
     return true;
 }
 

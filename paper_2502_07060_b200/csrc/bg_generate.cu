@@ -1,0 +1,357 @@
+// bg_generate.cu -- bg_generate(): the seeded phase-space generator ON THE DEVICE (SURVEY.md 8(f)
+// row f1; the paper prepares momenta and states on the host, and names offloading
+// that stage as possible future work).  One thread per phase-space point; the recipe is exactly
+// BASELINE.json:configs' generator as restated in DESIGN.md §4 (the host version is
+// paper_2502_07060_b200/inputs.py, which is this kernel's reference in the tests):
+//
+//   * counter-based RNG: draw c of point b, attempt a = SplitMix64 finaliser of key(seed,b,a) + c GOLDEN;
+//   * massless vectors from light-cone data: p- = -(sum_{mu>=2} g_mu p_mu^2)/(2 p+), p0 = p+ + p-/2,
+//     p1 = p+ - p-/2 (metric: PAPER.md:140, or the alternating one of PAPER.md:188);
+//   * p_1..p_{n-2} free, K = -sum p_i, q massless, p_{n-1} = alpha q with alpha = K^2/(2 K.q),
+//     p_n = K - p_{n-1};  eps_i = v_i - (v_i.p_i)/(r_i.p_i) r_i, or (d = 4) the spinor-helicity states
+//     eps_-(k;r) = vec(lam_k lamt_r^T)/[r k], eps_+(k;r) = 2 vec(lam_r lamt_k^T)/<r k> (Eq.(11));
+//   * F_p: points with K.q = 0, r_i.p_i = 0, a vanishing proper P_{i,j}^2 (or, with helicity states, a
+//     vanishing M00 of k_i or r_i) are redrawn with attempt + 1.
+//
+// Over F_p the output is bit-identical to inputs.py (exact arithmetic); over complex128 it agrees to
+// rounding (numpy sums and divides in its own order).  All inversions of a point go through
+// Montgomery's trick in three rounds (light-cone 1/(2p+), alpha, polarisation coefficients).
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <atomic>
+
+#include "../../include/bg.h"
+#include "bg_host_util.h"
+#include "bg_states.cuh"
+
+namespace {
+
+using bg::C128;
+using bg::Fp31;
+using bg::FpMont;
+
+constexpr uint64_t GOLDEN = 0x9E3779B97F4A7C15ull, M1 = 0xBF58476D1CE4E5B9ull, M2 = 0x94D049BB133111EBull;
+constexpr int kMaxAttempts = 64;
+
+__host__ __device__ inline uint64_t mix64(uint64_t z)
+{
+    z = (z ^ (z >> 30)) * M1;
+    z = (z ^ (z >> 27)) * M2;
+    return z ^ (z >> 31);
+}
+
+template <class F>
+struct GenParams {
+    typedef typename F::E E;
+    E* mom;                   // [batch][n][d]
+    E* pol;                   // [batch][n][d]
+    E* ref;                   // NULL or [batch][n][d]: the reference vectors r_i
+    unsigned long long* redraws;   // NULL or one device counter (incremented)
+    long long batch, start;
+    uint64_t seed;
+    int n, d, metric, row;    // row: padded elements per point in a shared-memory tile
+    int use_hel;
+    signed char hel[16];
+    uint32_t p;               // F_p: the prime
+    uint64_t rec_p, rec_pm1;  // floor((2^64-1)/p), floor((2^64-1)/(p-1))
+    bg::SpinorConsts<F> sc;
+    typename F::Params fld;
+};
+
+__device__ __forceinline__ uint32_t mod_u64(uint64_t u, uint32_t m, uint64_t rec)
+{   // u mod m with the precomputed reciprocal rec = floor((2^64-1)/m): the quotient estimate is at most 2 low
+    uint64_t r = u - __umul64hi(u, rec) * m;
+    while (r >= m) r -= m;
+    return (uint32_t)r;
+}
+
+// element e (0-based) of the point's stream: F_p uniform in [1,p) or in [0,p); complex (re, im) from two draws
+template <class F>
+struct Draws {
+    uint64_t key;
+    const GenParams<F>& prm;
+    const F& f;
+    __device__ __forceinline__ uint64_t draw(long long c) const { return mix64(key + (uint64_t)c * GOLDEN); }
+    __device__ __forceinline__ typename F::E nonzero(int e) const
+    {
+        if constexpr (F::kExact) return f.load_input(1u + mod_u64(draw(e + 1), prm.p - 1u, prm.rec_pm1));
+        else return any(e);
+    }
+    __device__ __forceinline__ typename F::E any(int e) const
+    {
+        if constexpr (F::kExact) {
+            return f.load_input(mod_u64(draw(e + 1), prm.p, prm.rec_p));
+        } else {
+            const double re = (double)(draw(2 * e + 1) >> 11) * 0x1p-52 - 1.0;
+            const double im = (double)(draw(2 * e + 2) >> 11) * 0x1p-52 - 1.0;
+            return make_double2(re, im);
+        }
+    }
+};
+
+template <class F>
+__device__ __forceinline__ typename F::E mdot(const F& f, int metric, int d, const typename F::E* x,
+                                              const typename F::E* y)
+{
+    typename F::A s = f.zero();
+    for (int mu = 0; mu < d; ++mu) {
+        const typename F::E xm = bg::metric_minus(metric, mu) ? f.neg(x[mu]) : x[mu];
+        s = f.relief(s);
+        s = f.mad(xm, f.canon(y[mu]), s);
+    }
+    return f.reduce(s);
+}
+
+// light-cone -> Cartesian: out[0..d) from p+ = stream element e0, p_perp = elements e0+1 .. e0+d-2,
+// inv2plus = 1/(2 p+)
+template <class F>
+__device__ __forceinline__ void massless(const F& f, const Draws<F>& dr, int metric, int d, int e0,
+                                         typename F::E inv2plus, typename F::E* out)
+{
+    typedef typename F::E E;
+    const E plus = dr.nonzero(e0);
+    E perp2 = f.ezero();
+    for (int mu = 2; mu < d; ++mu) {
+        const E x = dr.nonzero(e0 + mu - 1);
+        out[mu] = x;
+        const E sq = f.mul(x, x);
+        perp2 = bg::metric_minus(metric, mu) ? f.add(perp2, sq) : f.sub(perp2, sq);     // -(g_mu x^2)
+    }
+    const E half = f.mul(f.mul(perp2, inv2plus), f.half());      // p-/2
+    out[0] = f.add(plus, half);
+    out[1] = f.sub(plus, half);
+}
+
+template <class F>
+__global__ void generate_kernel(const GenParams<F> prm)
+{
+    typedef typename F::E E;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const F f(prm.fld, 0);
+    const int n = prm.n, d = prm.d, nd = n * d, metric = prm.metric, T = blockDim.x;
+    const int row = prm.row;                                   // >= nd, odd
+    E* tile_m = reinterpret_cast<E*>(smem_raw);                // [T][row] momenta
+    E* tile_p = tile_m + (size_t)T * row;                      // [T][row] v_i, then eps_i
+    E* tile_r = tile_p + (size_t)T * row;                      // [T][row] r_i
+    E* scr = tile_r + (size_t)T * row + (size_t)threadIdx.x * (4 * n + 2);   // [T][4n+2] inverses, dots
+    const long long tile0 = (long long)blockIdx.x * T;
+    const int valid = (int)min((long long)T, prm.batch - tile0);
+    const bool live = (int)threadIdx.x < valid;
+
+    if (live) {
+        E* km = tile_m + (size_t)threadIdx.x * row;
+        E* ep = tile_p + (size_t)threadIdx.x * row;
+        E* rr = tile_r + (size_t)threadIdx.x * row;
+        const uint64_t index = (uint64_t)(prm.start + tile0 + threadIdx.x);
+        const int eq = (n - 2) * (d - 1);                      // first stream element of q
+        const int ev = (n - 1) * (d - 1);                      // first stream element of the (v_i, r_i) block
+        int attempt = 0;
+        for (;; ++attempt) {
+            uint64_t key = mix64(prm.seed + GOLDEN);
+            key = mix64(key ^ (index * M1 + GOLDEN));
+            key = mix64(key ^ ((uint64_t)attempt * M2 + GOLDEN));
+            const Draws<F> dr{key, prm, f};
+            bool ok = true;
+            // ---- round A: 1/(2 p+) of every light-cone vector (free legs, q, r_1..r_n); p+ != 0 --------
+            E* invA = scr;                                     // [2n-1]
+            auto plus_elem = [&](int j) {
+                return j < n - 2 ? j * (d - 1) : j == n - 2 ? eq : ev + (j - (n - 1)) * (2 * d - 1) + d;
+            };
+            if constexpr (F::kExact) {
+                E c = f.one();
+                for (int j = 0; j < 2 * n - 1; ++j) {
+                    invA[j] = c;
+                    c = f.mul(c, f.dbl(dr.nonzero(plus_elem(j))));
+                }
+                E u = f.inv(c);
+                for (int j = 2 * n - 2; j >= 0; --j) {
+                    const E x = f.dbl(dr.nonzero(plus_elem(j)));
+                    invA[j] = f.mul(u, invA[j]);
+                    u = f.mul(u, x);
+                }
+            } else {
+                for (int j = 0; j < 2 * n - 1; ++j) invA[j] = f.inv(f.dbl(dr.nonzero(plus_elem(j))));
+            }
+            // ---- momenta ---------------------------------------------------------------------------------
+            E ksum[bg::kMaxD], q[bg::kMaxD];
+            for (int mu = 0; mu < d; ++mu) ksum[mu] = f.ezero();
+            for (int i = 0; i < n - 2; ++i) {
+                massless<F>(f, dr, metric, d, i * (d - 1), invA[i], km + i * d);
+                for (int mu = 0; mu < d; ++mu) ksum[mu] = f.add(ksum[mu], km[i * d + mu]);
+            }
+            massless<F>(f, dr, metric, d, eq, invA[n - 2], q);
+            for (int mu = 0; mu < d; ++mu) ksum[mu] = f.canon(f.neg(ksum[mu]));           // K
+            const E K2 = mdot<F>(f, metric, d, ksum, ksum), Kq = mdot<F>(f, metric, d, ksum, q);
+            if (F::kExact && f.is_zero(f.canon(Kq))) ok = false;
+            const E alpha = f.mul(K2, f.inv(f.dbl(Kq)));                                   // round B
+            for (int mu = 0; mu < d; ++mu) {
+                const E a = f.mul(alpha, q[mu]);
+                km[(n - 2) * d + mu] = a;
+                km[(n - 1) * d + mu] = f.sub(ksum[mu], a);
+            }
+            // ---- polarisations: v_i, r_i, then eps_i -----------------------------------------------------
+            E* den = scr + 2 * n;                              // [n]   r_i.p_i  (or the spinor denominators)
+            E* num = scr + 3 * n;                              // [n]   v_i.p_i
+            for (int i = 0; i < n; ++i) {
+                const int e0 = ev + i * (2 * d - 1);
+                for (int mu = 0; mu < d; ++mu) ep[i * d + mu] = dr.any(e0 + mu);
+                massless<F>(f, dr, metric, d, e0 + d, invA[n - 1 + i], rr + i * d);
+                const E rp = mdot<F>(f, metric, d, rr + i * d, km + i * d);
+                if (F::kExact && f.is_zero(f.canon(rp))) ok = false;
+                den[i] = rp;
+                num[i] = mdot<F>(f, metric, d, ep + i * d, km + i * d);
+            }
+            if (prm.use_hel) {
+                // spinor-helicity states on (k_i, r_i), unnormalised spinors (bg_states.cuh):
+                //   eps_- = vec(lam_k lamt'_r^T) M00(k) / [r k]',  eps_+ = 2 vec(lam_r lamt'_k^T) / (M00(k) <r k>)
+                for (int i = 0; i < n; ++i) {
+                    E lk[2], ltk[2], lr[2], ltr[2];
+                    bg::spinors_unnormalised<F>(f, prm.sc, km + i * d, lk, ltk);
+                    bg::spinors_unnormalised<F>(f, prm.sc, rr + i * d, lr, ltr);
+                    if (F::kExact && (f.is_zero(f.canon(lk[0])) || f.is_zero(f.canon(lr[0])))) ok = false;
+                    den[i] = prm.hel[i] < 0 ? f.sub(f.mul(ltr[0], ltk[1]), f.mul(ltr[1], ltk[0]))
+                                            : f.mul(lk[0], f.sub(f.mul(lr[0], lk[1]), f.mul(lr[1], lk[0])));
+                }
+            }
+            // round C: 1/den_i for all legs at once (zero-safe)
+            if constexpr (F::kExact) {
+                E* pre = scr;                                  // invA is no longer needed
+                E c = f.one();
+                for (int i = 0; i < n; ++i) {
+                    pre[i] = c;
+                    const bool z = f.is_zero(f.canon(den[i]));
+                    c = f.mul(c, z ? f.one() : den[i]);
+                }
+                E u = f.inv(c);
+                for (int i = n - 1; i >= 0; --i) {
+                    const bool z = f.is_zero(f.canon(den[i]));
+                    const E x = den[i];
+                    den[i] = z ? f.ezero() : f.mul(u, pre[i]);
+                    u = f.mul(u, z ? f.one() : x);
+                }
+            } else {
+                for (int i = 0; i < n; ++i) den[i] = f.inv(den[i]);
+            }
+            for (int i = 0; i < n; ++i) {
+                if (prm.use_hel) {
+                    E lk[2], ltk[2], lr[2], ltr[2], v4[4];
+                    bg::spinors_unnormalised<F>(f, prm.sc, km + i * d, lk, ltk);
+                    bg::spinors_unnormalised<F>(f, prm.sc, rr + i * d, lr, ltr);
+                    if (prm.hel[i] < 0) bg::bispinor_vec<F>(f, prm.sc, lk, ltr, f.mul(lk[0], den[i]), v4);
+                    else bg::bispinor_vec<F>(f, prm.sc, lr, ltk, f.dbl(den[i]), v4);
+                    for (int mu = 0; mu < 4; ++mu) ep[i * d + mu] = v4[mu];
+                } else {
+                    const E coef = f.mul(num[i], den[i]);
+                    for (int mu = 0; mu < d; ++mu)
+                        ep[i * d + mu] = f.sub(ep[i * d + mu], f.mul(coef, rr[i * d + mu]));
+                }
+            }
+            // ---- F_p: reject points with a vanishing proper invariant P_{i,j}^2 ------------------------------
+            if constexpr (F::kExact) {
+                const int m = n - 1;
+                for (int i = 0; i < m && ok; ++i) {
+                    E run[bg::kMaxD];
+                    for (int mu = 0; mu < d; ++mu) run[mu] = km[i * d + mu];
+                    for (int j = i + 1; j < m; ++j) {
+                        for (int mu = 0; mu < d; ++mu) run[mu] = f.canon(f.add(run[mu], km[j * d + mu]));
+                        if (i == 0 && j == m - 1) continue;
+                        if (f.is_zero(f.canon(mdot<F>(f, metric, d, run, run)))) ok = false;
+                    }
+                }
+            }
+            if (ok || !F::kExact || attempt + 1 >= kMaxAttempts) break;
+        }
+        if (attempt && prm.redraws) atomicAdd(prm.redraws, (unsigned long long)attempt);
+    }
+    __syncthreads();
+    // ---- coalesced stores of the three tiles ---------------------------------------------------------
+    const long long g0 = tile0 * nd;
+    for (int g = threadIdx.x; g < valid * nd; g += T) {
+        const int p = g / nd, w = g - p * nd;
+        prm.mom[g0 + g] = f.to_output(tile_m[(size_t)p * row + w]);
+        prm.pol[g0 + g] = f.to_output(tile_p[(size_t)p * row + w]);
+        if (prm.ref) prm.ref[g0 + g] = f.to_output(tile_r[(size_t)p * row + w]);
+    }
+}
+
+template <class F>
+int launch(const typename F::Params& fld, const bg::SpinorConsts<F>& sc, uint32_t p, int metric, int n, int d,
+           int64_t batch, uint64_t seed, int64_t start, const signed char* hel, void* mom, void* pol, void* ref,
+           unsigned long long* redraws, cudaStream_t stream)
+{
+    typedef typename F::E E;
+    GenParams<F> prm;
+    prm.mom = static_cast<E*>(mom);
+    prm.pol = static_cast<E*>(pol);
+    prm.ref = static_cast<E*>(ref);
+    prm.redraws = redraws;
+    prm.batch = batch;
+    prm.start = start;
+    prm.seed = seed;
+    prm.n = n; prm.d = d; prm.metric = metric;
+    prm.row = (n * d) | 1;
+    prm.use_hel = hel != nullptr;
+    for (int i = 0; i < 16; ++i) prm.hel[i] = hel && i < n ? hel[i] : 0;
+    prm.p = p;
+    prm.rec_p = p ? ~0ull / p : 0;
+    prm.rec_pm1 = p ? ~0ull / (p - 1u) : 0;
+    prm.sc = sc;
+    prm.fld = fld;
+    const size_t per_thread = ((size_t)3 * prm.row + 4 * n + 2) * sizeof(E);
+    int threads = 64;
+    while (threads > 8 && threads * per_thread > 200 * 1024) threads /= 2;
+    const size_t smem = threads * per_thread;
+    static std::atomic<uint64_t> attr_done{0};                 // bit i: attribute set on device i
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { cudaGetLastError(); return BG_ERR_CUDA; }
+    if (!(attr_done.load(std::memory_order_acquire) >> dev & 1ull)) {
+        if (cudaFuncSetAttribute(generate_kernel<F>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) !=
+            cudaSuccess) {
+            cudaGetLastError();
+            return BG_ERR_CUDA;
+        }
+        attr_done.fetch_or(1ull << dev, std::memory_order_release);
+    }
+    const int64_t blocks = (batch + threads - 1) / threads;
+    if (blocks > 0x7fffffffLL) return BG_ERR_ARG;
+    generate_kernel<F><<<(unsigned)blocks, threads, smem, stream>>>(prm);
+    return cudaGetLastError() == cudaSuccess ? BG_OK : BG_ERR_CUDA;
+}
+
+}  // namespace
+
+extern "C" int bg_generate(int field, uint32_t prime, int metric, int n, int d, int64_t batch, uint64_t seed,
+                           int64_t start, const signed char* helicities, void* momenta, void* polarisations,
+                           void* references, unsigned long long* redraws, cudaStream_t stream)
+{
+    if (n < 4 || n > 16 || d < 4 || d > 16 || batch < 0 || start < 0) return BG_ERR_ARG;
+    if (metric != BG_METRIC_MOSTLY_MINUS && metric != BG_METRIC_ALTERNATING) return BG_ERR_ARG;
+    if (helicities && d != 4) return BG_ERR_ARG;
+    if (batch == 0) return BG_OK;
+    if (!momenta || !polarisations || momenta == polarisations) return BG_ERR_ARG;
+    switch (field) {
+        case BG_FIELD_FP31: {
+            bg::SpinorConsts<Fp31> sc{0u, 0u};
+            if (helicities && !bg_spinor_consts_fp(bg::kP, metric, nullptr, &sc.jm, &sc.jv)) return BG_ERR_UNSUPPORTED;
+            return launch<Fp31>(Fp31::Params{}, sc, bg::kP, metric, n, d, batch, seed, start, helicities, momenta,
+                                polarisations, references, redraws, stream);
+        }
+        case BG_FIELD_FPMONT: {
+            FpMont::Params q{};
+            if (!bg_mont_constants(prime, 0, &q)) return BG_ERR_ARG;
+            bg::SpinorConsts<FpMont> sc{0u, 0u};
+            if (helicities && !bg_spinor_consts_fp(prime, metric, &q, &sc.jm, &sc.jv)) return BG_ERR_UNSUPPORTED;
+            return launch<FpMont>(q, sc, prime, metric, n, d, batch, seed, start, helicities, momenta, polarisations,
+                                  references, redraws, stream);
+        }
+        case BG_FIELD_C128: {
+            bg::SpinorConsts<C128> sc;
+            sc.jm = metric == BG_METRIC_MOSTLY_MINUS ? make_double2(0.0, 1.0) : make_double2(-1.0, 0.0);
+            sc.jv = metric == BG_METRIC_MOSTLY_MINUS ? make_double2(0.0, 1.0) : make_double2(1.0, 0.0);
+            return launch<C128>(C128::Params{}, sc, 0u, metric, n, d, batch, seed, start, helicities, momenta,
+                                polarisations, references, redraws, stream);
+        }
+    }
+    return BG_ERR_ARG;
+}

@@ -61,7 +61,7 @@ int launch(const typename F::Params& fld, int64_t batch, int states, int trees, 
 
 }  // namespace
 
-bool bg_mont_constants(uint32_t p, int i, bg::FpMont::Params* q);     // bg_api.cu
+#include "bg_host_util.h"
 
 extern "C" int bg_state_sum(int field, uint32_t prime, int64_t batch, int states, int trees,
                             const void* const* amps, void* out, cudaStream_t stream)
