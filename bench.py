@@ -16,8 +16,12 @@ Printed: ONE JSON line (rank 0) with the contract keys plus `roofline` (bound "a
 modmul-bound line of SURVEY.md §8(d) / DESIGN.md §Roofline), `cpu_baseline` (the oracle as
 it stands, on this box's host cores, on a bounded sample), `e2e` (the same metric through
 `bg_amplitudes_host` with pinned HOST buffers, H2D/D2H copies inside the timed region),
-`clocks`, `gpu_launches`, and `per_config` (short device-resident timings of the other
-BASELINE.json configs, N=1 only; `--headline-only` skips them).
+`clocks`, `gpu_launches`, `per_config` (short device-resident timings of the other BASELINE.json
+configs, each with its own oracle timing and, for complex128, the branch statistics of tolerance
+rule R9), `features` (the SURVEY.md 8(f) rows: state configurations, generic prime, alternating
+metric, colour orderings, state sum, device generator and states, the general kernel) and
+`e2e_seeded` (seed -> amplitudes on the host with the generator on the device); N=1 only,
+`--headline-only` skips them.
 `--impl reference` times the CPU oracle alone (this tier's reference arm).
 """
 from __future__ import annotations
@@ -47,9 +51,24 @@ UNIT = "amplitudes/s"
 SM_COUNT = 148
 WIDE_MUL_LANES_PER_CLK_PER_SM = 32
 DFMA_LANES_PER_CLK_PER_SM = 64      # checked against the DFMA probe
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the recursion kernel, from the committed
-# `ncu --set full` capture (profiles/r01b_cfg2_metrics.txt); algorithmic bytes are 407 MB
-NCU_TRAFFIC_BYTES = {"cfg2": 410.2e6}
+
+
+def ncu_traffic(name: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the config's kernel, parsed from the
+    committed `ncu --set full` summary that profiles/traffic.json names for it (None if there is none)"""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            fn = json.load(f)[name]
+        unit = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+        tot = 0.0
+        with open(os.path.join(ROOT, "profiles", fn)) as f:
+            for line in f:
+                t = line.split()
+                if len(t) == 3 and t[0] in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+                    tot += float(t[1]) * unit[t[2]]
+        return {"bytes": tot, "source": "profiles/" + fn} if tot else None
+    except Exception:  # noqa: BLE001
+        return None
 
 
 def log(*a):
@@ -120,6 +139,9 @@ def op_counts(field: str, n: int, d: int) -> dict:
     R = m * (m - 1) // 2 - 1
     w = 4 if field == "fp31" else 16
     return {"mul_ref": 6 * d * comb(n, 3) + 6 * d * comb(n, 4) + d * R + 3 * (R - 1) + d * R + d,
+            # what the kernels' factored form executes (bg.h: bg_opcount_t.mul_factored)
+            "mul_exec": 6 * d * comb(n, 3) + 2 * d * comb(n, 4) + (R + 1) * (d + 1) + 2 * d * R + d + m * d + d * R +
+            3 * (R - 1) + 38,
             "bytes": 2 * n * d * w + w}
 
 
@@ -264,6 +286,172 @@ def e2e_bench(binding, torch, name: str, mom: np.ndarray, pol: np.ndarray, steps
     return {"s_per_step": dt / steps, "h2d": int(mom.nbytes + pol.nbytes), "d2h": int(ho.nbytes), "out": res}
 
 
+def time_device(torch, launch, steps: int, warmup: int = 3) -> float:
+    """median duration in ms of `steps` launches (CUDA events on the current stream)"""
+    stream = torch.cuda.current_stream()
+    for _ in range(warmup):
+        launch()
+    torch.cuda.synchronize()
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    evs[0].record(stream)
+    for k in range(steps):
+        launch()
+        evs[k + 1].record(stream)
+    torch.cuda.synchronize()
+    return statistics.median(evs[k].elapsed_time(evs[k + 1]) for k in range(steps))
+
+
+def oracle_baseline(name: str, cores: int, target_s: float) -> dict:
+    """the oracle as it stands on `cores` threads, on the first points of the config's workload"""
+    sample = pick_oracle_sample(name, cores, target_s)
+    t = time_oracle(name, sample, cores)[0]
+    return {"value": sample / t, "unit": UNIT, "cores": cores, "kind": "naive oracle (literal Eq.(6), % p arithmetic, "
+            "one Fermat inverse per propagator)", "sample": f"the first {sample} points of {name}, one pass, {t:.2f} s"}
+
+
+def r9_report(name: str, got, points: int) -> dict:
+    """branch statistics of tolerance rule R9 (oracle/rule.py) on the first `points` points of a complex config"""
+    from oracle import rule
+    mom, pol, _ = inputs.make_config_threaded(name, batch=points)
+    ok, st = rule.check(got[:points], rule.evaluate(mom, pol, threads=host_cores()))
+    st["all_pass"] = bool(ok.all())
+    return st
+
+
+def run_features(binding, torch, steps: int) -> list:
+    """SURVEY.md 8(f) rows, device-resident timings (inputs from the device generator)"""
+    B = binding
+    s = torch.cuda.current_stream().cuda_stream
+    rows = []
+    n, d = 8, 6
+    prime = 2147483629                       # 2^31 - 19
+
+    def ev(pb, batch, mom, pol, out):
+        rc = B.bg_evaluate(pb, batch, mom.data_ptr(), pol.data_ptr(), out.data_ptr(), None, None, s)
+        if rc != B.BG_OK:
+            raise RuntimeError(B.bg_status_string(rc))
+
+    def row(name, amps, ms, **kw):
+        rows.append({"feature": name, "value": amps / (ms * 1e-3), "unit": UNIT, "kernel_ms_median": ms, **kw})
+
+    # f2: S state configurations per momentum point (Eq.(4)); the same 2^20 amplitudes per launch for every S
+    for S in (1, 4, 16):
+        batch = (1 << 20) // S
+        mom, pol0, _ = B.generate(B.FIELD_FP31, n, d, batch, seed=0)
+        pol = torch.stack([pol0] + [B.generate(B.FIELD_FP31, n, d, batch, seed=s_)[1] for s_ in range(1, S)],
+                          dim=1).contiguous()
+        out = torch.empty((batch, S), dtype=torch.int32, device="cuda")
+        pb = B.problem(B.FIELD_FP31, n, d, states=S)
+        ms = time_device(torch, lambda: ev(pb, batch, mom, pol, out), steps)
+        row(f"f2 states: n=8 d=6 F_p, {batch} points x S={S}", batch * S, ms,
+            input_bytes_per_amplitude=(1 + S) * n * d * 4 / S)
+    del pol, pol0
+    # f3: generic 31-bit prime (Montgomery), alternating metric, four primes in one launch
+    batch = 1 << 20
+    mom, pol, _ = B.generate(B.FIELD_FPMONT, n, d, batch, seed=0, prime=prime)
+    out = torch.empty(batch, dtype=torch.int32, device="cuda")
+    pb = B.problem(B.FIELD_FPMONT, n, d, primes=(prime,))
+    row(f"f3 generic prime p=2^31-19 (Montgomery): n=8 d=6, 2^20 points", batch,
+        time_device(torch, lambda: ev(pb, batch, mom, pol, out), steps))
+    mom, pol, _ = B.generate(B.FIELD_FP31, n, d, batch, seed=0, metric=1)
+    pb = B.problem(B.FIELD_FP31, n, d, metric=1)
+    row("f3 alternating metric: n=8 d=6 F_p(2^31-1), 2^20 points", batch,
+        time_device(torch, lambda: ev(pb, batch, mom, pol, out), steps))
+    primes = (prime, 2013265921, 1073741827, (1 << 31) - 1)
+    bq = 1 << 18
+    gens = [B.generate(B.FIELD_FPMONT, n, d, bq, seed=0, prime=p) for p in primes]
+    mom4 = torch.stack([g[0] for g in gens]).contiguous()
+    pol4 = torch.stack([g[1] for g in gens]).contiguous()
+    out4 = torch.empty((4, bq), dtype=torch.int32, device="cuda")
+    pb = B.problem(B.FIELD_FPMONT, n, d, primes=primes)
+    row("f3 four primes in one launch: n=8 d=6, 4 x 2^18 points", 4 * bq,
+        time_device(torch, lambda: ev(pb, bq, mom4, pol4, out4), steps))
+    del gens, mom4, pol4
+    # f4: K colour orderings per point (Eq.(5))
+    K, bo = 24, 1 << 15
+    rng = np.random.default_rng(0)
+    perms = np.array([list(rng.permutation(n - 1)) + [n - 1] for _ in range(K)], dtype=np.uint8)
+    dperm = torch.from_numpy(perms).cuda()
+    mom, pol, _ = B.generate(B.FIELD_FP31, n, d, bo, seed=0)
+    outk = torch.empty((bo, K), dtype=torch.int32, device="cuda")
+    pb = B.problem(B.FIELD_FP31, n, d, n_orderings=K, orderings_ptr=dperm.data_ptr())
+    row(f"f4 colour orderings: n=8 d=6 F_p, 2^15 points x K={K}", bo * K,
+        time_device(torch, lambda: ev(pb, bo, mom, pol, outk), steps))
+    # the general kernel (shapes outside the compiled grid): the performance cliff bg.h documents
+    for (gn, gd, gb) in ((11, 5, 1 << 16), (16, 4, 1 << 14)):
+        mom, pol, _ = B.generate(B.FIELD_FP31, gn, gd, gb, seed=0)
+        outg = torch.empty(gb, dtype=torch.int32, device="cuda")
+        pb = B.problem(B.FIELD_FP31, gn, gd)
+        ms = time_device(torch, lambda: ev(pb, gb, mom, pol, outg), max(3, steps // 4))
+        oc = op_counts("fp31", gn, gd)
+        row(f"general kernel: n={gn} d={gd} F_p, {gb} points", gb, ms,
+            roofline_frac=oc["mul_ref"] * gb / (ms * 1e-3) / (SM_COUNT * WIDE_MUL_LANES_PER_CLK_PER_SM * 1.965e9),
+            kernel=B.bg_kernel_info(B.FIELD_FP31, gn, gd))
+    # Eq.(4) state sum: HBM-bound
+    T, S, bs = 2, 16, 1 << 20
+    amps = [torch.randint(0, 2 ** 31 - 1, (bs, S), dtype=torch.int32, device="cuda") for _ in range(T)]
+    outs = torch.empty(bs, dtype=torch.int32, device="cuda")
+    ms = time_device(torch, lambda: B.bg_state_sum(B.FIELD_FP31, 0, bs, S, [a.data_ptr() for a in amps],
+                                                   outs.data_ptr(), s), steps)
+    rows.append({"feature": f"f2 state sum (Eq.(4)): {T} trees x S={S}, 2^20 points", "value": bs / (ms * 1e-3),
+                 "unit": "points/s", "kernel_ms_median": ms, "hbm_GBs": (T * S + 1) * 4 * bs / (ms * 1e-3) / 1e9,
+                 "hbm_frac": (T * S + 1) * 4 * bs / (ms * 1e-3) / 1e9 / hbm_peak()})
+    # f1: generator and states on the device
+    gb = 1 << 20
+    mom = torch.empty((gb, n, d), dtype=torch.int32, device="cuda")
+    pol = torch.empty_like(mom)
+    ms = time_device(torch, lambda: B.bg_generate(B.FIELD_FP31, 0, 0, n, d, gb, 0, 0, None, mom.data_ptr(),
+                                                  pol.data_ptr(), None, None, s), steps)
+    rows.append({"feature": "f1 device generator: n=8 d=6 F_p, 2^20 points", "value": gb / (ms * 1e-3),
+                 "unit": "points/s", "kernel_ms_median": ms, "hbm_frac": 2 * n * d * 4 * gb / (ms * 1e-3) / 1e9 / hbm_peak()})
+    momA, _, refA, _ = B.generate(B.FIELD_FP31, n, d, 1 << 17, seed=0, metric=1, want_references=True)
+    chi = B.generate(B.FIELD_FP31, n, 4, 1 << 17, seed=1, metric=1, want_references=True)[2]
+    kv, cv = momA.reshape(-1, d), chi.reshape(-1, 4).contiguous()
+    eps = torch.empty((kv.shape[0], d - 2, d), dtype=torch.int32, device="cuda")
+    til = torch.empty_like(eps)
+    ms = time_device(torch, lambda: B.bg_states(B.FIELD_FP31, 0, 1, d, kv.shape[0], kv.data_ptr(), cv.data_ptr(),
+                                                eps.data_ptr(), til.data_ptr(), None, s), steps)
+    rows.append({"feature": "f1 device states (Eqs.(8)-(18)): d=6 alternating metric F_p, 2^20 vectors",
+                 "value": kv.shape[0] / (ms * 1e-3), "unit": "vectors/s", "kernel_ms_median": ms})
+    return rows
+
+
+def seeded_e2e(binding, torch, name: str, steps: int) -> dict:
+    """seed -> amplitudes in HOST memory: bg_generate + bg_amplitudes on the device, one D2H copy of the results
+    per step (no input ever crosses the host link).  Wall clock, synchronised on both sides."""
+    cfg = inputs.CONFIGS[name]
+    B = binding
+    n, d, batch = cfg["n"], cfg["d"], cfg["batch"]
+    field = B.FIELD_FP31 if cfg["field"] == "fp31" else B.FIELD_C128
+    dt = torch.int32 if cfg["field"] == "fp31" else torch.complex128
+    mom = torch.empty((batch, n, d), dtype=dt, device="cuda")
+    pol = torch.empty_like(mom)
+    out = torch.empty(batch, dtype=dt, device="cuda")
+    host = torch.empty(batch, dtype=dt).pin_memory()
+    s = torch.cuda.current_stream().cuda_stream
+    hel = cfg["helicities"]
+
+    def step(k):
+        rc = B.bg_generate(field, 0, 0, n, d, batch, 0, 0, hel, mom.data_ptr(), pol.data_ptr(), None, None, s)
+        rc = rc or B.bg_amplitudes(field, n, d, batch, mom.data_ptr(), pol.data_ptr(), out.data_ptr(), s)
+        if rc != B.BG_OK:
+            raise RuntimeError(B.bg_status_string(rc))
+        host.copy_(out, non_blocking=True)
+
+    for k in range(2):
+        step(k)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for k in range(steps):
+        step(k)
+    torch.cuda.synchronize()
+    dt_s = (time.perf_counter() - t0) / steps
+    return {"value": batch / dt_s, "unit": UNIT, "ms_per_step": dt_s * 1e3, "h2d_bytes_per_step": 0,
+            "d2h_bytes_per_step": int(host.numel() * host.element_size()), "steps": steps,
+            "api": "bg_generate (seeded kinematics on the device, SURVEY.md 8(f) f1) + bg_amplitudes + D2H of the results",
+            "result": host.numpy().view(np.uint32).copy() if cfg["field"] == "fp31" else host.numpy().copy()}
+
+
 def roofline(field: str, n: int, d: int, batch: int, kernel_ms: float, sm_max_mhz: float, probes: dict | None,
              traffic):
     oc = op_counts(field, n, d)
@@ -279,14 +467,22 @@ def roofline(field: str, n: int, d: int, batch: int, kernel_ms: float, sm_max_mh
         achieved = 4 * oc["mul_ref"] * batch / (kernel_ms * 1e-3)
         unit, what = "GDFMA/s", ("4 DFMA per complex multiply-add x M_ref x points / kernel time; peak = "
                                  "FP64-pipe issue rate at max SM clock (DESIGN.md §Roofline)")
+    executed = (1 if field == "fp31" else 4) * oc["mul_exec"] * batch / (kernel_ms * 1e-3)
     r = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": unit, "frac": achieved / peak,
-         "traffic": traffic, "peak_source": "derived from unit counts and clock (DESIGN.md §7), confirmed by the on-box probe; MEASURED_PEAKS.json has no ALU peak",
+         "traffic": None if traffic is None else traffic["bytes"],
+         "traffic_source": None if traffic is None else traffic["source"],
+         "basis": "frac = EFFECTIVE work: the literal Eq.(6) count M_ref (algorithmic, SURVEY.md 8(d)) / time / peak; "
+                  "frac_executed = the multiplications the factored kernels actually issue (mul_exec) / time / peak, "
+                  "i.e. multiplier-pipe utilisation",
+         "executed": executed / 1e9, "frac_executed": executed / peak, "mul_exec_per_amplitude": oc["mul_exec"],
+         "peak_source": "derived from unit counts and clock (DESIGN.md §7), confirmed by the on-box probe; MEASURED_PEAKS.json has no ALU peak",
          "what": what, "mul_ref_per_amplitude": oc["mul_ref"], "kernel_ms": kernel_ms,
          "hbm_frac": oc["bytes"] * batch / (kernel_ms * 1e-3) / 1e9 / hbm_peak()}
     if probes:
         key = "imad_wide_rz" if field == "fp31" else "dfma"       # the bare multiplier rate / the DFMA rate
         r["probe_peak"] = probes[key]["ops_per_s"] / 1e9
         r["frac_of_probe"] = achieved / probes[key]["ops_per_s"]
+        r["frac_executed_of_probe"] = executed / probes[key]["ops_per_s"]
         if field == "fp31":
             # north_star's line: canonical Mersenne-31 modular multiplications per second (R_mm, measured)
             r["modmul_line_Gmodmul_s"] = probes["modmul"]["ops_per_s"] / 1e9
@@ -380,7 +576,7 @@ def run_gpu(args) -> None:
                 str(n): round(smsp_hz / (probes[k]["ops_per_s"] / (n + 1) / 32), 2)
                 for n, k in ((1, "mix"), (2, "mix2"), (3, "mix3"))}
         line["roofline"] = roofline(cfg["field"], cfg["n"], cfg["d"], batch, kernel_ms, clocks.get("sm_max_mhz"),
-                                    probes, args.traffic if name == "cfg2" else None)
+                                    probes, ncu_traffic(name))
         if world == 1 and not args.headline_only:
             per = []
             for other in inputs.CONFIGS:
@@ -390,11 +586,25 @@ def run_gpu(args) -> None:
                 r = device_bench(binding, torch, other, oc["batch"], 0, args.config_steps, 3, None)
                 kms = statistics.median(r["per_launch_ms"])
                 rl = roofline(oc["field"], oc["n"], oc["d"], oc["batch"], kms, clocks.get("sm_max_mhz"), probes, None)
-                per.append({"workload": workload_name(other), "value": oc["batch"] / (kms * 1e-3), "unit": UNIT,
-                            "kernel_ms_median": kms, "launches": args.config_steps,
-                            "roofline_frac": rl["frac"], "roofline_unit": rl["unit"], "hbm_frac": rl["hbm_frac"]})
+                entry = {"workload": workload_name(other), "value": oc["batch"] / (kms * 1e-3), "unit": UNIT,
+                         "kernel_ms_median": kms, "launches": args.config_steps,
+                         "roofline_frac": rl["frac"], "roofline_frac_executed": rl["frac_executed"],
+                         "roofline_unit": rl["unit"], "hbm_frac": rl["hbm_frac"],
+                         "kernel": binding.bg_kernel_info(binding.FIELD_FP31 if oc["field"] == "fp31" else
+                                                          binding.FIELD_C128, oc["n"], oc["d"])}
+                if not args.no_cpu_baseline:
+                    entry["cpu_baseline"] = oracle_baseline(other, host_cores(), 2.0)
+                    if oc["field"] == "c128":
+                        pts = min(oc["batch"], 1 << 17) if oc["n"] <= 6 else 4096
+                        entry["parity_rule_R9"] = r9_report(other, binding.to_numpy(r["out"]), pts)
+                per.append(entry)
                 del r
             line["per_config"] = per
+            line["features"] = run_features(binding, torch, args.config_steps)
+            se = seeded_e2e(binding, torch, name, e2e_steps)
+            se["matches_device_path"] = bool(np.array_equal(se.pop("result"), binding.to_numpy(res["out"]))) \
+                if cfg["field"] == "fp31" else None
+            line["e2e_seeded"] = se
         if world == 1 and not args.no_cpu_baseline:
             cores = host_cores()
             sample = args.oracle_points or pick_oracle_sample(name, cores, 10.0)
@@ -404,7 +614,12 @@ def run_gpu(args) -> None:
             t = sum(ts)
             line["cpu_baseline"] = {"value": sample * len(ts) / t, "unit": UNIT, "cores": cores, "kind": "oracle",
                                     "sample": f"the first {sample} points of {name} (same seeded workload), "
-                                              f"{len(ts)} passes, {t:.1f} s on {cores} threads"}
+                                              f"{len(ts)} passes, {t:.1f} s on {cores} threads",
+                                    "note": "the oracle is deliberately naive (literal Eq.(6), % p arithmetic, one "
+                                            "Fermat inverse per propagator): a reported baseline, not a tuned CPU code"}
+            t1c = time_oracle(name, 1 << 14, 1)[0]
+            line["cpu_baseline"]["single_core"] = {"value": (1 << 14) / t1c, "unit": UNIT, "cores": 1,
+                                                   "sample": f"the first 16384 points of {name}, {t1c:.2f} s"}
         print(json.dumps(line))
     if dist is not None:
         dist.barrier()
@@ -425,9 +640,6 @@ def main():
     ap.add_argument("--headline-only", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-probes", action="store_true")
-    ap.add_argument("--traffic", type=float, default=NCU_TRAFFIC_BYTES.get("cfg2"),
-                    help="dram bytes per launch of the recursion kernel from the committed ncu capture "
-                         "(profiles/); reported as roofline.traffic")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         log("[bench] note: fewer than 3 warm-up steps requested")

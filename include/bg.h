@@ -114,11 +114,15 @@ typedef struct {
     int states;              /* S */
     int n_primes;
     uint32_t primes[BG_MAX_PRIMES];
+    int n_orderings;         /* K colour orderings per point (Eq.(5)); 0 or 1: the caller's order */
+    const unsigned char* orderings;   /* NULL, or DEVICE [K][n]: row o lists, for positions 1..n, which of the
+                                caller's legs (0-based) stands there; every row must be a permutation of
+                                0..n-1 (not checked: entries >= n are clamped to n-1) */
 } bg_problem_t;
 
-/* momenta [P][batch][n][d], polarisations [P][batch][S][n][d], out [P][batch][S], status NULL or
- * [P][batch] (P = max(1, n_primes)); currents NULL, or [batch][m][m][d] when S == 1 and P == 1.
- * Device pointers, asynchronous on `stream`. */
+/* momenta [P][batch][n][d], polarisations [P][batch][S][n][d], out [P][batch][K][S], status NULL or
+ * [P][batch] (P = max(1, n_primes), K = max(1, n_orderings)); currents NULL, or [batch][m][m][d] when
+ * S == 1, P == 1 and K == 1.  Device pointers, asynchronous on `stream`. */
 int bg_evaluate(const bg_problem_t* problem, int64_t batch, const void* momenta, const void* polarisations,
                 void* out, void* currents, uint32_t* status, cudaStream_t stream);
 
@@ -126,6 +130,15 @@ int bg_evaluate(const bg_problem_t* problem, int64_t batch, const void* momenta,
  * polarisations [batch][S][n][d], out [batch][S]. */
 int bg_amplitudes_states(int field, int n, int d, int64_t batch, int states, const void* momenta,
                          const void* polarisations, void* out, uint32_t* status, cudaStream_t stream);
+
+/* K colour orderings of every point in one launch: the colour-ordered amplitudes C(sigma_o(1), .., sigma_o(n))
+ * that the colour decomposition Eq.(5), sums over the permutations P(1..n-1) with the
+ * traces Tr(T^a_sigma(1) .. T^a_n).  The inputs of a point are read from HBM once; every ordering re-stages
+ * them in its order (rows a1-a6 per ordering).  orderings: DEVICE [K][n] as in bg_problem_t; out [batch][K];
+ * status bit0 = some proper P^2 vanished in SOME ordering.  Mostly-minus metric. */
+int bg_amplitudes_orderings(int field, int n, int d, int64_t batch, int n_orderings, const unsigned char* orderings,
+                            const void* momenta, const void* polarisations, void* out, uint32_t* status,
+                            cudaStream_t stream);
 
 /* Several generic 31-bit primes in one launch (Q-reconstruction from the F_p values);
  * momenta, polarisations [n_primes][batch][n][d] residues mod primes[q], out [n_primes][batch]. */

@@ -111,6 +111,17 @@ def evaluate(field: int, momenta: np.ndarray, polarisations: np.ndarray, metric:
     return res[0] if len(res) == 1 else tuple(res)
 
 
+def orderings(field: int, momenta: np.ndarray, polarisations: np.ndarray, perms, metric: int = MOSTLY_MINUS,
+              prime: int = 0, threads: int = 1) -> np.ndarray:
+    """The colour-ordered amplitudes C(sigma(1), .., sigma(n)) of Eq.(5), for every
+    row sigma of perms [K, n] (0-based legs): the literal recursion run once per ordering on the
+    permuted inputs, nothing shared.  Returns out [batch, K] (or [batch, K, S] with a state axis)."""
+    perms = np.asarray(perms)
+    outs = [evaluate(field, momenta[:, list(s)], polarisations[..., list(s), :], metric, prime, threads=threads)
+            for s in perms]
+    return np.stack(outs, axis=1)
+
+
 def amplitudes(field: int, momenta: np.ndarray, polarisations: np.ndarray,
                want_currents: bool = False, want_status: bool = False, threads: int = 1):
     """evaluate() with the mostly-minus metric, p = 2^31-1 and one state configuration"""

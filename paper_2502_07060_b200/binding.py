@@ -26,7 +26,7 @@ PEAK_KINDS = {"imad_wide": 0, "imad": 1, "alu": 2, "mix": 3, "modmul": 4, "dfma"
 P31 = (1 << 31) - 1
 
 EXPORTS = ["bg_amplitudes", "bg_amplitudes_status", "bg_currents", "bg_evaluate", "bg_amplitudes_states",
-           "bg_amplitudes_primes", "bg_state_sum", "bg_states", "bg_generate", "bg_amplitudes_host", "bg_host_workspace_bytes", "bg_modulus",
+           "bg_amplitudes_primes", "bg_amplitudes_orderings", "bg_state_sum", "bg_states", "bg_generate", "bg_amplitudes_host", "bg_host_workspace_bytes", "bg_modulus",
            "bg_status_string", "bg_version", "bg_op_count", "bg_kernel_info", "bg_kernel_info_problem",
            "bg_set_kernel_override", "bg_peak_probe", "bg_selftest_schedules"]
 
@@ -44,13 +44,16 @@ class OpCount(ctypes.Structure):
 class Problem(ctypes.Structure):
     """bg_problem_t"""
     _fields_ = [("field", ctypes.c_int), ("metric", ctypes.c_int), ("n", ctypes.c_int), ("d", ctypes.c_int),
-                ("states", ctypes.c_int), ("n_primes", ctypes.c_int), ("primes", ctypes.c_uint32 * MAX_PRIMES)]
+                ("states", ctypes.c_int), ("n_primes", ctypes.c_int), ("primes", ctypes.c_uint32 * MAX_PRIMES),
+                ("n_orderings", ctypes.c_int), ("orderings", ctypes.c_void_p)]
 
 
-def problem(field, n, d, metric=METRIC_MOSTLY_MINUS, states=1, primes=()) -> Problem:
+def problem(field, n, d, metric=METRIC_MOSTLY_MINUS, states=1, primes=(), n_orderings=0, orderings_ptr=None) -> Problem:
     pb = Problem(field, metric, n, d, states, len(primes))
     for i, p in enumerate(primes):
         pb.primes[i] = p
+    pb.n_orderings = n_orderings
+    pb.orderings = orderings_ptr
     return pb
 
 
@@ -92,6 +95,8 @@ def load(rebuild_if_stale: bool = False):
     lib.bg_generate.argtypes = [ci, ctypes.c_uint32, ci, ci, ci, i64, ctypes.c_uint64, i64, ctypes.c_char_p, vp, vp, vp,
                                 vp, vp]
     lib.bg_generate.restype = ci
+    lib.bg_amplitudes_orderings.argtypes = [ci, ci, ci, i64, ci, vp, vp, vp, vp, vp, vp]
+    lib.bg_amplitudes_orderings.restype = ci
     lib.bg_kernel_info_problem.argtypes = [ctypes.POINTER(Problem), ctypes.POINTER(KernelInfo)]
     lib.bg_set_kernel_override.argtypes = [ci, ci]
     lib.bg_amplitudes_host.argtypes = [ci, ci, ci, i64, vp, vp, vp, vp, vp, sz]
@@ -151,6 +156,12 @@ def bg_amplitudes_primes(metric, n, d, batch, primes, momenta_ptr, polarisations
     arr = (ctypes.c_uint32 * len(primes))(*primes)
     return load().bg_amplitudes_primes(metric, n, d, batch, len(primes), arr, momenta_ptr, polarisations_ptr,
                                        out_ptr, status_ptr, stream_ptr)
+
+
+def bg_amplitudes_orderings(field, n, d, batch, n_orderings, orderings_ptr, momenta_ptr, polarisations_ptr, out_ptr,
+                            status_ptr=None, stream_ptr=0):
+    return load().bg_amplitudes_orderings(field, n, d, batch, n_orderings, orderings_ptr, momenta_ptr,
+                                          polarisations_ptr, out_ptr, status_ptr, stream_ptr)
 
 
 def bg_state_sum(field, prime, batch, states, amp_ptrs, out_ptr, stream_ptr=0):
@@ -286,10 +297,19 @@ def amplitudes(momenta, polarisations, out=None, status=None, stream=None):
     return out
 
 
-def evaluate(momenta, polarisations, metric=METRIC_MOSTLY_MINUS, primes=(), status=None, stream=None):
+def evaluate(momenta, polarisations, metric=METRIC_MOSTLY_MINUS, primes=(), status=None, stream=None,
+             orderings=None):
     """The generalised path (bg_evaluate).  momenta [B,n,d] (with primes: [P,B,n,d]); polarisations the same
-    shape, or with a state axis [B,S,n,d] ([P,B,S,n,d]).  Returns out [B] / [B,S] (leading [P] with primes)."""
+    shape, or with a state axis [B,S,n,d] ([P,B,S,n,d]); orderings: None or a [K,n] array of leg permutations
+    (Eq.(5)).  Returns out [B] / [B,S] / [B,K] / [B,K,S] (leading [P] with primes)."""
     torch = _torch()
+    ord_dev = None
+    if orderings is not None:
+        o = np.ascontiguousarray(orderings, dtype=np.uint8)
+        if o.ndim != 2 or o.shape[1] != momenta.shape[-2] or \
+                not (np.sort(o, axis=1) == np.arange(o.shape[1], dtype=np.uint8)).all():
+            raise BgError("orderings must be [K, n] permutations of 0..n-1")
+        ord_dev = torch.from_numpy(o).to(momenta.device)
     lead = 1 if primes else 0
     if momenta.dim() != 3 + lead or polarisations.dim() not in (3 + lead, 4 + lead):
         raise BgError("bad tensor ranks for evaluate()")
@@ -301,9 +321,11 @@ def evaluate(momenta, polarisations, metric=METRIC_MOSTLY_MINUS, primes=(), stat
     field = FIELD_FPMONT if primes else field_of(momenta)
     if primes and (field_of(momenta) != FIELD_FP31 or momenta.shape[0] != len(primes)):
         raise BgError("with primes the inputs are uint32/int32 residues with a leading [len(primes)] axis")
-    shape = ([len(primes)] if primes else []) + [batch] + ([states] if has_states else [])
+    shape = ([len(primes)] if primes else []) + [batch] + ([ord_dev.shape[0]] if ord_dev is not None else []) + \
+        ([states] if has_states else [])
     out = torch.empty(shape, dtype=momenta.dtype, device=momenta.device)
-    pb = problem(field, n, d, metric, states, tuple(primes))
+    pb = problem(field, n, d, metric, states, tuple(primes), 0 if ord_dev is None else int(ord_dev.shape[0]),
+                 None if ord_dev is None else ord_dev.data_ptr())
     s = (stream or torch.cuda.current_stream(momenta.device)).cuda_stream
     with torch.cuda.device(momenta.device):
         _check(bg_evaluate(pb, batch, momenta.data_ptr(), polarisations.data_ptr(), out.data_ptr(), None,

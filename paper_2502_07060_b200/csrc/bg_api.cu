@@ -261,6 +261,8 @@ int launch_typed(Launch* L, const bg_problem_t& pb, const typename F::Params& fl
     prm.status = status;
     prm.batch = batch;
     prm.states = pb.states;
+    prm.n_orderings = pb.n_orderings > 1 || pb.orderings ? (pb.n_orderings < 1 ? 1 : pb.n_orderings) : 1;
+    prm.orderings = pb.orderings;
     prm.n = pb.n;
     prm.stride = L->stride;
     prm.fld = fld;
@@ -283,6 +285,7 @@ int check_problem(const bg_problem_t* pb)
     int rc = check_shape(pb->field, pb->metric, pb->n, pb->d);
     if (rc != BG_OK) return rc;
     if (pb->states < 1 || pb->states > 65535) return BG_ERR_ARG;
+    if (pb->n_orderings < 0 || pb->n_orderings > (1 << 24) || (pb->n_orderings > 1 && !pb->orderings)) return BG_ERR_ARG;
     if (pb->field == BG_FIELD_FPMONT) {
         if (pb->n_primes < 1 || pb->n_primes > BG_MAX_PRIMES) return BG_ERR_ARG;
     } else if (pb->n_primes != 0) {
@@ -301,7 +304,7 @@ int run(const bg_problem_t& pb, int64_t batch, const void* mom, const void* pol,
         for (int i = 0; i < pb.n_primes; ++i)
             if (!bg_mont_constants(pb.primes[i], i, &mont)) return BG_ERR_ARG;
     Launch* L = nullptr;
-    rc = select(pb.field, pb.metric, pb.n, pb.d, pb.states > 1, &L);
+    rc = select(pb.field, pb.metric, pb.n, pb.d, pb.states > 1 || pb.orderings, &L);
     if (rc != BG_OK) return rc;
     if (batch < 0) return BG_ERR_ARG;
     if (batch == 0) return BG_OK;
@@ -310,7 +313,7 @@ int run(const bg_problem_t& pb, int64_t batch, const void* mom, const void* pol,
         (reinterpret_cast<uintptr_t>(status) & 3u))
         return BG_ERR_ARG;
     if (out == mom || out == pol) return BG_ERR_ARG;
-    if (cur && (pb.states != 1 || pb.n_primes > 1)) return BG_ERR_ARG;
+    if (cur && (pb.states != 1 || pb.n_primes > 1 || pb.orderings)) return BG_ERR_ARG;
     switch (pb.field) {
         case BG_FIELD_FP31: return launch_typed<Fp31>(L, pb, Fp31::Params{}, batch, mom, pol, out, cur, status, stream);
         case BG_FIELD_C128: return launch_typed<C128>(L, pb, C128::Params{}, batch, mom, pol, out, cur, status, stream);
@@ -402,6 +405,17 @@ int bg_amplitudes_states(int field, int n, int d, int64_t batch, int states, con
     if (field == BG_FIELD_FPMONT) return BG_ERR_ARG;
     return run(simple_problem(field, BG_METRIC_MOSTLY_MINUS, n, d, states), batch, momenta, polarisations, out,
                nullptr, status, stream);
+}
+
+int bg_amplitudes_orderings(int field, int n, int d, int64_t batch, int n_orderings, const unsigned char* orderings,
+                            const void* momenta, const void* polarisations, void* out, uint32_t* status,
+                            cudaStream_t stream)
+{
+    if (field == BG_FIELD_FPMONT || n_orderings < 1 || !orderings) return BG_ERR_ARG;
+    bg_problem_t pb = simple_problem(field, BG_METRIC_MOSTLY_MINUS, n, d, 1);
+    pb.n_orderings = n_orderings;
+    pb.orderings = orderings;
+    return run(pb, batch, momenta, polarisations, out, nullptr, status, stream);
 }
 
 int bg_amplitudes_primes(int metric, int n, int d, int64_t batch, int n_primes, const uint32_t* primes,
@@ -538,7 +552,7 @@ int bg_kernel_info_problem(const bg_problem_t* problem, bg_kernel_info_t* out)
     int rc = check_problem(problem);
     if (rc != BG_OK) return rc;
     Launch* L = nullptr;
-    rc = select(problem->field, problem->metric, problem->n, problem->d, problem->states > 1, &L);
+    rc = select(problem->field, problem->metric, problem->n, problem->d, problem->states > 1 || problem->orderings, &L);
     if (rc != BG_OK) return rc;
     out->specialised = L->kind == BG_KIND_GENERAL ? 0 : 1 + L->kind;
     out->threads_per_block = L->threads;

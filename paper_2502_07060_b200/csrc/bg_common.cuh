@@ -25,11 +25,13 @@ struct BgParams {
     typedef typename F::E E;
     const E* mom;         // [primes][batch][n][D]
     const E* pol;         // [primes][batch][states][n][D]
-    E* out;               // [primes][batch][states]
+    E* out;               // [primes][batch][orderings][states]
     E* currents;          // NULL or [batch][m][m][D]   (states == 1, one prime)
     uint32_t* status;     // NULL or [primes][batch]
     long long batch;
     int states;           // S >= 1 polarisation configurations per momentum point (Eq.(4))
+    int n_orderings;      // K >= 1 colour orderings per point (Eq.(5))
+    const unsigned char* orderings;   // NULL (K == 1, the caller's order) or device [K][n]: leg at position i
     int n;                // general kernel only
     int stride;           // general kernel only: record stride in elements
     typename F::Params fld;

@@ -67,18 +67,25 @@ __global__ void bg_general_kernel(const BgParams<F> prm)
     E* Wt = rec + lay.off_w;
     const int R = lay.r;
 
+    uint32_t status = 0;
+    const int n_ord = prm.n_orderings;
+    for (int o = 0; o < n_ord; ++o) {
+    // colour ordering o (Eq.(5)): the inputs are staged in that order, the rest is unchanged
+    const unsigned char* perm = prm.orderings ? prm.orderings + o * n : nullptr;
+    if (o > 0) __syncthreads();
     // ---- a0: stage the momenta k_1..k_m into the PS rows 1..m, coalesced ---------------------------
     {
         const E* gm = prm.mom + (pbase + tile0) * nd;
         const int per = m * D, total = valid * per;
         for (int g = threadIdx.x; g < total; g += T) {
             const int p = g / per, w = g - p * per;
-            smem[(size_t)p * stride + (lay.ps0 + 1) * D + w] = f.load_input(gm[(long long)p * nd + w]);
+            const int row = w / D, c = w - row * D;
+            const int srow = perm ? min((int)perm[row], n - 1) : row;
+            smem[(size_t)p * stride + (lay.ps0 + 1) * D + w] = f.load_input(gm[(long long)p * nd + srow * D + c]);
         }
     }
     __syncthreads();
 
-    uint32_t status = 0;
     if (live) {
         // ---- a1: doubled prefix sums (Eq.(7)) ----------------------------------------
         E run[D];
@@ -141,7 +148,9 @@ __global__ void bg_general_kernel(const BgParams<F> prm)
             const int total = valid * nd;
             for (int g = threadIdx.x; g < total; g += T) {
                 const int p = g / nd, w = g - p * nd;
-                smem[(size_t)p * stride + w] = f.load_input(gp[(long long)p * states * nd + w]);
+                const int row = w / D, c = w - row * D;
+                const int srow = perm ? min((int)perm[row], n - 1) : row;
+                smem[(size_t)p * stride + w] = f.load_input(gp[(long long)p * states * nd + srow * D + c]);
             }
         }
         __syncthreads();
@@ -237,7 +246,7 @@ __global__ void bg_general_kernel(const BgParams<F> prm)
                     ld_vec<F, D>(rec + m * D, e);
                     lower_neg<F, MET, D>(f, 0, e, ne);
                     const E nout = f.reduce(dot_plain<F, D>(f, ne, v));
-                    prm.out[(pbase + pt) * states + s] = f.to_output(f.neg(nout));
+                    prm.out[((pbase + pt) * n_ord + o) * states + s] = f.to_output(f.neg(nout));
                 }
                 if (prm.currents) {
                     E* dst = prm.currents + (pt * m * m + (long long)(i - 1) * m + (i + L - 2)) * D;
@@ -251,6 +260,7 @@ __global__ void bg_general_kernel(const BgParams<F> prm)
                 E* dst = prm.currents + (pt * m * m + (long long)c * m + c) * D;
                 for (int mu = 0; mu < D; ++mu) dst[mu] = f.to_output(rec[c * D + mu]);
             }
+    }
     }
 }
 

@@ -85,20 +85,31 @@ struct TileLane {
 // a0: stage rows of the tile's points from global memory (coalesced, one vector unit per thread and
 // step).  src: first element of point tile0's block; a point's block is ND elements, consecutive
 // points are `pstride` elements apart; the first ROWS rows go to record rows [ROW0, ROW0 + ROWS).
+// perm: NULL, or the colour ordering (Eq.(5)): record row ROW0 + i receives the caller's row perm[i].
 template <class F, int N, int D, int W, int S, int ROW0, int ROWS>
 __device__ __forceinline__ void tile_stage(const F& f, const TileLane<F, N, D, W, S>& t, const typename F::E* src,
-                                           long long pstride)
+                                           long long pstride, const unsigned char* __restrict__ perm)
 {
     typedef TileCfg<F, N, D, W, S> C;
     typedef typename VecType<F, C::U>::type V;
     constexpr int U = C::U, row0 = ROW0;
     constexpr int upp = ROWS * D / U;                           // units per point
+    constexpr int upr = D / U;                                  // units per row
     const int total = t.valid * upp;
+    if (perm == nullptr) {
 #pragma unroll 4
-    for (int g = threadIdx.x; g < total; g += 32 * W) {
-        const int p = g / upp, u = g - p * upp;
-        V* r = reinterpret_cast<V*>(t.vec + (size_t)p * C::VSTRIDE) + row0 * D / U;
-        r[u] = load_unit<F>(f, __ldg(reinterpret_cast<const V*>(src + p * pstride) + u));
+        for (int g = threadIdx.x; g < total; g += 32 * W) {
+            const int p = g / upp, u = g - p * upp;
+            V* r = reinterpret_cast<V*>(t.vec + (size_t)p * C::VSTRIDE) + row0 * D / U;
+            r[u] = load_unit<F>(f, __ldg(reinterpret_cast<const V*>(src + p * pstride) + u));
+        }
+    } else {
+#pragma unroll 2
+        for (int g = threadIdx.x; g < total; g += 32 * W) {
+            const int p = g / upp, u = g - p * upp, row = u / upr, c = u - row * upr;
+            V* r = reinterpret_cast<V*>(t.vec + (size_t)p * C::VSTRIDE) + row0 * D / U;
+            r[u] = load_unit<F>(f, __ldg(reinterpret_cast<const V*>(src + p * pstride) + min((int)__ldg(perm + row), N - 1) * upr + c));
+        }
     }
 }
 

@@ -228,28 +228,34 @@ __global__ void __launch_bounds__(32 * W) bg_unit_kernel(const BgParams<F> prm)
     t.valid = (int)min((long long)TP, prm.batch - t.tile0);
     t.pt = t.tile0 + t.point;
     t.live = t.point < t.valid;
-    const int states = prm.states;
+    const int states = prm.states, n_ord = prm.n_orderings;
     const long long pbase = t.q * prm.batch;                  // first point of this prime's arrays
     const E* gmom = prm.mom + (pbase + t.tile0) * ND;
     const E* gpol = prm.pol + (pbase + t.tile0) * states * ND;
-    E* gout = prm.out + (pbase + t.pt) * states;
+    E* gout = prm.out + (pbase + t.pt) * n_ord * states;
     uint32_t* gstat = prm.status ? prm.status + pbase : nullptr;
 
-    // ---- a0: stage the momenta k_1..k_m (k_n is never used) and the first state configuration ----
     if (threadIdx.x < TP) t.stat[threadIdx.x] = 0;
-    tile_stage<F, N, D, W, S, Setup::PARK, M>(f, t, gmom, ND);
-    tile_stage<F, N, D, W, S, 0, N>(f, t, gpol, (long long)states * ND);
-    __syncthreads();
-    // ---- a1-a3: prefix sums, invariants, propagators (momenta only: once per tile) ----------------
-    Setup::template momenta<MET>(f, t, gstat);
-
     E* rec = t.rec();
     E* sc = t.sc();
+#pragma unroll 1
+    for (int o = 0; o < n_ord; ++o, gout += states) {
+    // colour ordering o (Eq.(5)): the inputs are re-staged in that order (from L2 after the
+    // first pass) and everything below runs unchanged
+    const unsigned char* perm = prm.orderings ? prm.orderings + o * N : nullptr;
+    if (o > 0) __syncthreads();                                // the previous sweep is done with the record
+    // ---- a0: stage the momenta k_1..k_m (k_n is never used) and the first state configuration ----
+    tile_stage<F, N, D, W, S, Setup::PARK, M>(f, t, gmom, ND, perm);
+    tile_stage<F, N, D, W, S, 0, N>(f, t, gpol, (long long)states * ND, perm);
+    __syncthreads();
+    // ---- a1-a3: prefix sums, invariants, propagators (momenta only: once per tile and ordering) ----
+    Setup::template momenta<MET>(f, t, gstat);
+
 #pragma unroll 1
     for (int s = 0; s < states; ++s) {
         if (s > 0) {
             __syncthreads();                                   // the previous sweep is done with eps_n
-            tile_stage<F, N, D, W, S, 0, N>(f, t, gpol + (long long)s * ND, (long long)states * ND);
+            tile_stage<F, N, D, W, S, 0, N>(f, t, gpol + (long long)s * ND, (long long)states * ND, perm);
             __syncthreads();
         }
         Setup::template singles<MET>(f, t, prm.currents);
@@ -309,6 +315,7 @@ __global__ void __launch_bounds__(32 * W) bg_unit_kernel(const BgParams<F> prm)
             }
             if (L < M) __syncthreads();
         }
+    }
     }
 }
 

@@ -273,3 +273,65 @@ def test_state_sum_argument_checks(bgl):
     assert bgl.bg_state_sum(3, 0, 8, 4, [p], p + 2048) == bgl.BG_ERR_ARG
     assert bgl.bg_state_sum(0, 0, 0, 4, [p], p + 2048) == bgl.BG_OK
     torch.cuda.synchronize()
+
+
+# ---- K colour orderings per point (Eq.(5)) -----------------------------------------------
+def _perms(n, K, seed):
+    """K orderings: the identity, the cyclic shift, the reflection, the U(1) insertions of leg 0, then random"""
+    rng = np.random.default_rng(seed)
+    ident = list(range(n))
+    out = [ident, ident[1:] + ident[:1], ident[::-1]]
+    out += [ident[1:][:pos] + [0] + ident[1:][pos:] for pos in range(n - 1)]
+    while len(out) < K:
+        out.append(list(rng.permutation(n - 1)) + [n - 1])
+    return np.array(out[:max(K, n + 2)], dtype=np.uint8)
+
+
+@pytest.mark.parametrize("n,d,batch", [(8, 6, 70), (6, 4, 133), (12, 6, 33), (7, 5, 45), (5, 7, 40)], ids=lambda v: str(v))
+def test_orderings_fp(bgl, oracle_mod, n, d, batch):
+    import torch
+    perms = _perms(n, 24, n)
+    mom, pol, _ = inputs.make_fp_inputs(n, d, batch, seed=17)
+    mom = mom.copy()
+    mom[2, 2] = mom[2, 1]                             # k_2 = k_3 at point 2: singular in the orderings where they touch
+    status = torch.zeros(batch, dtype=torch.int32, device="cuda")
+    got = bgl.to_numpy(bgl.evaluate(bgl.to_device(mom), bgl.to_device(pol), orderings=perms, status=status))
+    torch.cuda.synchronize()
+    ref = oracle_mod.orderings(oracle_mod.FP31, mom, pol, perms, threads=8)
+    assert got.shape == (batch, len(perms)) and np.array_equal(got, ref)
+    st = status.cpu().numpy()
+    assert st[2] == 1 and st.sum() == 1
+    ok = np.arange(batch) != 2
+    # what the colour-ordered amplitudes must obey (pins of the oracle, here straight from the kernels):
+    g = got[ok].astype(np.int64)
+    assert np.array_equal(g[:, 1], g[:, 0])                                              # cyclicity
+    assert np.array_equal(g[:, 2], g[:, 0] if n % 2 == 0 else (P31 - g[:, 0]) % P31)     # reflection
+    assert not (g[:, 3:3 + n - 1].sum(axis=1) % P31).any()                               # U(1) decoupling
+
+
+def test_orderings_entry_point_states_and_complex(bgl, oracle_mod):
+    import torch
+    from oracle import rule
+    n, d, batch, S = 6, 6, 40, 3
+    perms = _perms(n, 12, 3)
+    mom, pol, _ = inputs.make_state_inputs("fp31", n, d, batch, S, seed=19)
+    got = bgl.to_numpy(bgl.evaluate(bgl.to_device(mom), bgl.to_device(pol), orderings=perms))
+    torch.cuda.synchronize()
+    assert got.shape == (batch, len(perms), S)
+    assert np.array_equal(got, oracle_mod.orderings(oracle_mod.FP31, mom, pol, perms, threads=8))
+    # the named entry point
+    dm, dp = bgl.to_device(mom), bgl.to_device(np.ascontiguousarray(pol[:, 0]))
+    dperm = torch.from_numpy(perms).cuda()
+    out = torch.empty((batch, len(perms)), dtype=torch.int32, device="cuda")
+    rc = bgl.bg_amplitudes_orderings(bgl.FIELD_FP31, n, d, batch, len(perms), dperm.data_ptr(), dm.data_ptr(),
+                                     dp.data_ptr(), out.data_ptr(), None, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert rc == bgl.BG_OK and np.array_equal(bgl.to_numpy(out), got[:, :, 0])
+    # complex128 (cfg1 shape: bg_reg_kernel cannot loop over orderings, the two-lane tiled kernel runs)
+    mom, pol, _ = inputs.make_complex_inputs(6, 4, 64, seed=5, helicities=(-1, -1, 1, 1, 1, 1))
+    perms = _perms(6, 10, 4)
+    got = bgl.to_numpy(bgl.evaluate(bgl.to_device(mom), bgl.to_device(pol), orderings=perms))
+    torch.cuda.synchronize()
+    for o, s in enumerate(perms):
+        ok, st = rule.check(got[:, o], rule.evaluate(mom[:, list(s)], pol[:, list(s)], threads=8))
+        assert ok.all(), (o, st)

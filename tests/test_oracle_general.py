@@ -222,3 +222,19 @@ def test_states_equal_independent_calls(oracle_mod, field):
         o1, c1 = oracle_mod.amplitudes(f, mom, pols[s], want_currents=True)
         assert np.array_equal(out[:, s], o1) and np.array_equal(cur[:, s], c1)
     assert not st.any()
+
+
+# ------------------------------------------------------------------ colour orderings
+def test_orderings_are_independent_calls_and_obey_the_identities(oracle_mod):
+    """oracle.orderings (Eq.(5)) = one literal evaluation per ordering; the sum over the
+    n-1 insertions of leg 1 vanishes (U(1) decoupling), cyclic shifts agree"""
+    n, d = 6, 5
+    mom, pol, _ = inputs.make_fp_inputs(n, d, 10, seed=6)
+    ident = list(range(n))
+    perms = [ident, ident[2:] + ident[:2]] + [ident[1:][:pos] + [0] + ident[1:][pos:] for pos in range(n - 1)]
+    out = oracle_mod.orderings(oracle_mod.FP31, mom, pol, perms)
+    assert out.shape == (10, len(perms))
+    for o, s in enumerate(perms):
+        assert np.array_equal(out[:, o], oracle_mod.amplitudes(oracle_mod.FP31, mom[:, s], pol[:, s]))
+    assert np.array_equal(out[:, 0], out[:, 1])
+    assert not (out[:, 2:].astype(np.int64).sum(axis=1) % P31).any()
