@@ -76,7 +76,7 @@ const KernelEntry* find_entry(int field, int metric, int n, int d, bool multi_st
             const KernelEntry& e = t[i];
             if (e.field != field || e.metric != metric || e.n != n || e.d != d) continue;
             if (e.smem > (size_t)kMaxSmemPerBlock) continue;
-            if (multi_state && e.kind == BG_KIND_REG) continue;         // bg_reg_kernel: one configuration only
+            if (multi_state && !e.func_multi) continue;                 // bg_reg_kernel: one configuration only
             if (want_kind >= 0 && e.kind != want_kind) continue;
             if (!first) first = &e;
             if (want_w == 0 || e.w == want_w) return &e;
@@ -112,9 +112,9 @@ int fill_general(int field, int metric, int n, int d, Launch* L)
     return BG_OK;
 }
 
-void fill_entry(const KernelEntry& e, Launch* L)
+void fill_entry(const KernelEntry& e, bool multi, Launch* L)
 {
-    L->func = e.func;
+    L->func = multi ? e.func_multi : e.func;
     L->kind = e.kind;
     L->threads = 32 * e.w;
     L->points_per_block = e.tp;
@@ -149,10 +149,10 @@ int select(int field, int metric, int n, int d, bool multi_state, Launch** out)
             const KernelEntry* e = ok == 0 ? nullptr
                                            : find_entry(field, metric, n, d, multi_state, ok - 1, ow);
             int rc = BG_OK;
-            if (e) fill_entry(*e, &g_over);
+            if (e) fill_entry(*e, multi_state, &g_over);
             else if (ok == 0 || !(e = find_entry(field, metric, n, d, multi_state, -1, 0)))
                 rc = fill_general(field, metric, n, d, &g_over);
-            else fill_entry(*e, &g_over);
+            else fill_entry(*e, multi_state, &g_over);
             if (rc != BG_OK) { g_over_key[0] = -2; return rc; }
             memcpy(g_over_key, key, sizeof(key));
         }
@@ -167,7 +167,7 @@ int select(int field, int metric, int n, int d, bool multi_state, Launch** out)
         s = st.load(std::memory_order_relaxed);
         if (s == 0) {
             int rc = BG_OK;
-            if (const KernelEntry* e = find_entry(field, metric, n, d, multi_state, -1, 0)) fill_entry(*e, L);
+            if (const KernelEntry* e = find_entry(field, metric, n, d, multi_state, -1, 0)) fill_entry(*e, multi_state, L);
             else rc = fill_general(field, metric, n, d, L);
             s = rc == BG_OK ? 1 : 2;
             st.store(s, std::memory_order_release);

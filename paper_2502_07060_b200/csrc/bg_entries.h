@@ -17,7 +17,8 @@ struct KernelEntry {
     int w;                   // warps per tile (bg_reg_kernel: independent warps per block)
     int kind;                // BgKernelKind
     int tp;                  // points per block
-    const void* func;
+    const void* func;        // one state configuration, one ordering
+    const void* func_multi;  // loops over orderings and state configurations; NULL: not available (bg_reg_kernel)
     size_t smem;
 };
 

@@ -8,5 +8,5 @@ BG_DEFINE_TABLE(metric,
     unit_entry<Fp31, ALT, 10, 8, 8>(),
     unit_entry<Fp31, ALT, 12, 6, 8>(),
     unit_entry<C128, ALT, 6, 4, 2, 2>(),
-    unit_entry<C128, ALT, 12, 6, 16, 2>(),
+    unit_entry<C128, ALT, 12, 6, 8, 2>(),
 )

@@ -46,6 +46,12 @@ struct TileCfg {
     static constexpr int NSCAL = SC_SCR + NSLOTS * (D + 1);
     static constexpr int THREADS = 32 * W;
     static constexpr size_t SMEM_BYTES = (size_t)TP * (VSTRIDE + NSCAL) * sizeof(E) + TP * sizeof(uint32_t);
+    // resident blocks per SM that shared memory allows (228 KB per SM, 1 KB reserved per block): the register
+    // budget of the kernel is set so that registers do not lower it (__launch_bounds__ in bg_unit.cuh)
+    static constexpr int SMEM_BLOCKS = (int)(233472 / (SMEM_BYTES + 1024)) < 1 ? 1 : (int)(233472 / (SMEM_BYTES + 1024));
+    static constexpr int WARP_BLOCKS = 64 / W;                 // 64 resident warps per SM
+    static constexpr int MIN_BLOCKS = SMEM_BLOCKS < WARP_BLOCKS ? (SMEM_BLOCKS > 16 ? 16 : SMEM_BLOCKS)
+                                                                : (WARP_BLOCKS > 16 ? 16 : WARP_BLOCKS);
 };
 
 // proper multi-gluon range r (level-major) -> lo | hi << 8 with P_{i,j} = PS_hi - PS_lo

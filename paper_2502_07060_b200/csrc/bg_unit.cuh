@@ -199,8 +199,12 @@ __device__ __forceinline__ void unit_finish(const F& f, const TileLane<F, N, D, 
     }
 }
 
-template <class F, int MET, int N, int D, int W, int S>
-__global__ void __launch_bounds__(32 * W) bg_unit_kernel(const BgParams<F> prm)
+// MULTI = false: one state configuration and one colour ordering per point, no loops around the sweep (the
+// headline path).  MULTI = true adds the loops over orderings and state configurations; it is a separate
+// instantiation because ptxas stops using the uniform datapath for the control flow and the table loads of
+// the sweep once it sits inside another loop (+12 % executed instructions, measured on cfg3).
+template <class F, int MET, int N, int D, int W, int S, bool MULTI>
+__global__ void __launch_bounds__(32 * W, TileCfg<F, N, D, W, S>::MIN_BLOCKS) bg_unit_kernel(const BgParams<F> prm)
 {
     typedef TileCfg<F, N, D, W, S> C;
     typedef TileSetup<F, N, D, W, S> Setup;
@@ -219,30 +223,33 @@ __global__ void __launch_bounds__(32 * W) bg_unit_kernel(const BgParams<F> prm)
     // the warp index, broadcast from lane 0 so that everything derived from it (task bounds,
     // task words, branch conditions) is compiled as warp-uniform
     const int lane = threadIdx.x & 31;
-    t.warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
-    t.point = lane & (TP - 1);
-    t.half = lane / TP;
-    t.mu0 = t.half * DL;
+    const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
+    t.warp = warp;
+    t.point = S == 1 ? lane : lane & (TP - 1);
+    t.half = S == 1 ? 0 : lane / TP;
+    t.mu0 = S == 1 ? 0 : t.half * DL;
     t.q = blockIdx.y;
     t.tile0 = (long long)blockIdx.x * TP;
     t.valid = (int)min((long long)TP, prm.batch - t.tile0);
     t.pt = t.tile0 + t.point;
     t.live = t.point < t.valid;
-    const int states = prm.states, n_ord = prm.n_orderings;
+    const int states = MULTI ? prm.states : 1, n_ord = MULTI ? prm.n_orderings : 1;
     const long long pbase = t.q * prm.batch;                  // first point of this prime's arrays
     const E* gmom = prm.mom + (pbase + t.tile0) * ND;
     const E* gpol = prm.pol + (pbase + t.tile0) * states * ND;
     E* gout = prm.out + (pbase + t.pt) * n_ord * states;
     uint32_t* gstat = prm.status ? prm.status + pbase : nullptr;
 
-    if (threadIdx.x < TP) t.stat[threadIdx.x] = 0;
+    // (a warp-uniform condition first: after a thread-divergent branch in front of the barriers ptxas no longer
+    // treats the sweep as convergent and gives up the uniform datapath for its control flow and table loads)
+    if (warp == 0 && lane < TP) t.stat[lane] = 0;
     E* rec = t.rec();
     E* sc = t.sc();
 #pragma unroll 1
     for (int o = 0; o < n_ord; ++o, gout += states) {
     // colour ordering o (Eq.(5)): the inputs are re-staged in that order (from L2 after the
     // first pass) and everything below runs unchanged
-    const unsigned char* perm = prm.orderings ? prm.orderings + o * N : nullptr;
+    const unsigned char* perm = MULTI && prm.orderings ? prm.orderings + o * N : nullptr;
     if (o > 0) __syncthreads();                                // the previous sweep is done with the record
     // ---- a0: stage the momenta k_1..k_m (k_n is never used) and the first state configuration ----
     tile_stage<F, N, D, W, S, Setup::PARK, M>(f, t, gmom, ND, perm);
@@ -266,7 +273,7 @@ __global__ void __launch_bounds__(32 * W) bg_unit_kernel(const BgParams<F> prm)
         for (int L = 2; L <= M; ++L) {
             const int lbase = UnitTable<N>::index(L, 1);
             const int own = ut.u[lbase].own, widx = ut.u[lbase].w;
-            const int t0 = tb.beg[L][t.warp], t1 = tb.beg[L][t.warp + 1];
+            const int t0 = tb.beg[L][warp], t1 = tb.beg[L][warp + 1];
 #pragma unroll 1
             for (int k = t0; k < t1; ++k) {
                 const uint32_t ta = tb.task[k].a;

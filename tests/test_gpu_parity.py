@@ -243,7 +243,7 @@ VARIANTS = [("fp31", 8, 6, "unit1", 4), ("fp31", 8, 6, "unit1", 6), ("fp31", 8, 
             ("fp31", 8, 6, "general", 0), ("fp31", 12, 6, "general", 0), ("c128", 6, 4, "general", 0),
             ("c128", 6, 4, "reg", 4), ("c128", 6, 4, "unit2", 2), ("c128", 6, 4, "unit2", 4),
             ("c128", 6, 4, "unit1", 2), ("c128", 6, 4, "unit1", 4),
-            ("c128", 12, 6, "unit2", 16), ("c128", 12, 6, "unit2", 8),
+            ("c128", 12, 6, "unit2", 16), ("c128", 12, 6, "unit2", 8), ("c128", 12, 6, "unit2", 4),
             # the shapes of the paper's own benchmarks (bg_inst_paper.cu)
             ("fp31", 6, 4, "unit1", 2), ("fp31", 8, 4, "unit1", 4), ("fp31", 9, 4, "unit1", 4), ("fp31", 6, 6, "unit1", 2),
             ("fp31", 9, 6, "unit1", 4), ("fp31", 6, 8, "unit1", 2), ("fp31", 8, 8, "unit1", 4), ("fp31", 9, 8, "unit1", 4),
