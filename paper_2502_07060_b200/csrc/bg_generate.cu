@@ -19,8 +19,6 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#include <atomic>
-
 #include "../../include/bg.h"
 #include "bg_host_util.h"
 #include "bg_states.cuh"
@@ -50,7 +48,7 @@ struct GenParams {
     unsigned long long* redraws;   // NULL or one device counter (incremented)
     long long batch, start;
     uint64_t seed;
-    int n, d, metric, row;    // row: padded elements per point in a shared-memory tile
+    int n, d, metric;
     int use_hel;
     signed char hel[16];
     uint32_t p;               // F_p: the prime
@@ -123,27 +121,21 @@ __device__ __forceinline__ void massless(const F& f, const Draws<F>& dr, int met
     out[1] = f.sub(plus, half);
 }
 
-template <class F>
-__global__ void generate_kernel(const GenParams<F> prm)
+// The point's vectors live in thread-local arrays (local memory is interleaved by thread, so the same element of
+// neighbouring points is contiguous: conflict-free, cached in L1/L2) -- shared-memory tiles limited the kernel to
+// 256 resident threads per SM, and its long dependent chains (three field inversions per point) need many more.
+template <class F, int MAXND>
+__global__ void __launch_bounds__(128) generate_kernel(const GenParams<F> prm)
 {
     typedef typename F::E E;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
     const F f(prm.fld, 0);
-    const int n = prm.n, d = prm.d, nd = n * d, metric = prm.metric, T = blockDim.x;
-    const int row = prm.row;                                   // >= nd, odd
-    E* tile_m = reinterpret_cast<E*>(smem_raw);                // [T][row] momenta
-    E* tile_p = tile_m + (size_t)T * row;                      // [T][row] v_i, then eps_i
-    E* tile_r = tile_p + (size_t)T * row;                      // [T][row] r_i
-    E* scr = tile_r + (size_t)T * row + (size_t)threadIdx.x * (4 * n + 2);   // [T][4n+2] inverses, dots
-    const long long tile0 = (long long)blockIdx.x * T;
-    const int valid = (int)min((long long)T, prm.batch - tile0);
-    const bool live = (int)threadIdx.x < valid;
+    const int n = prm.n, d = prm.d, nd = n * d, metric = prm.metric;
+    const long long pt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = pt < prm.batch;
 
     if (live) {
-        E* km = tile_m + (size_t)threadIdx.x * row;
-        E* ep = tile_p + (size_t)threadIdx.x * row;
-        E* rr = tile_r + (size_t)threadIdx.x * row;
-        const uint64_t index = (uint64_t)(prm.start + tile0 + threadIdx.x);
+        E km[MAXND], ep[MAXND], rr[MAXND], scr[4 * 16 + 2];    // momenta; v_i then eps_i; r_i; inverses and dots
+        const uint64_t index = (uint64_t)(prm.start + pt);
         const int eq = (n - 2) * (d - 1);                      // first stream element of q
         const int ev = (n - 1) * (d - 1);                      // first stream element of the (v_i, r_i) block
         int attempt = 0;
@@ -263,15 +255,17 @@ __global__ void generate_kernel(const GenParams<F> prm)
             if (ok || !F::kExact || attempt + 1 >= kMaxAttempts) break;
         }
         if (attempt && prm.redraws) atomicAdd(prm.redraws, (unsigned long long)attempt);
-    }
-    __syncthreads();
-    // ---- coalesced stores of the three tiles ---------------------------------------------------------
-    const long long g0 = tile0 * nd;
-    for (int g = threadIdx.x; g < valid * nd; g += T) {
-        const int p = g / nd, w = g - p * nd;
-        prm.mom[g0 + g] = f.to_output(tile_m[(size_t)p * row + w]);
-        prm.pol[g0 + g] = f.to_output(tile_p[(size_t)p * row + w]);
-        if (prm.ref) prm.ref[g0 + g] = f.to_output(tile_r[(size_t)p * row + w]);
+        // every thread stores its own point (n d contiguous elements per array; L2 merges the sectors)
+        E* gm = prm.mom + pt * nd;
+        E* gp = prm.pol + pt * nd;
+        for (int w = 0; w < nd; ++w) {
+            gm[w] = f.to_output(km[w]);
+            gp[w] = f.to_output(ep[w]);
+        }
+        if (prm.ref) {
+            E* gr = prm.ref + pt * nd;
+            for (int w = 0; w < nd; ++w) gr[w] = f.to_output(rr[w]);
+        }
     }
 }
 
@@ -290,7 +284,6 @@ int launch(const typename F::Params& fld, const bg::SpinorConsts<F>& sc, uint32_
     prm.start = start;
     prm.seed = seed;
     prm.n = n; prm.d = d; prm.metric = metric;
-    prm.row = (n * d) | 1;
     prm.use_hel = hel != nullptr;
     for (int i = 0; i < 16; ++i) prm.hel[i] = hel && i < n ? hel[i] : 0;
     prm.p = p;
@@ -298,24 +291,12 @@ int launch(const typename F::Params& fld, const bg::SpinorConsts<F>& sc, uint32_
     prm.rec_pm1 = p ? ~0ull / (p - 1u) : 0;
     prm.sc = sc;
     prm.fld = fld;
-    const size_t per_thread = ((size_t)3 * prm.row + 4 * n + 2) * sizeof(E);
-    int threads = 64;
-    while (threads > 8 && threads * per_thread > 200 * 1024) threads /= 2;
-    const size_t smem = threads * per_thread;
-    static std::atomic<uint64_t> attr_done{0};                 // bit i: attribute set on device i
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { cudaGetLastError(); return BG_ERR_CUDA; }
-    if (!(attr_done.load(std::memory_order_acquire) >> dev & 1ull)) {
-        if (cudaFuncSetAttribute(generate_kernel<F>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) !=
-            cudaSuccess) {
-            cudaGetLastError();
-            return BG_ERR_CUDA;
-        }
-        attr_done.fetch_or(1ull << dev, std::memory_order_release);
-    }
-    const int64_t blocks = (batch + threads - 1) / threads;
+    const int64_t blocks = (batch + 127) / 128;
     if (blocks > 0x7fffffffLL) return BG_ERR_ARG;
-    generate_kernel<F><<<(unsigned)blocks, threads, smem, stream>>>(prm);
+    const int nd = n * d;
+    if (nd <= 64) generate_kernel<F, 64><<<(unsigned)blocks, 128, 0, stream>>>(prm);
+    else if (nd <= 128) generate_kernel<F, 128><<<(unsigned)blocks, 128, 0, stream>>>(prm);
+    else generate_kernel<F, 256><<<(unsigned)blocks, 128, 0, stream>>>(prm);
     return cudaGetLastError() == cudaSuccess ? BG_OK : BG_ERR_CUDA;
 }
 

@@ -119,9 +119,10 @@ __device__ __forceinline__ void tile_stage(const F& f, const TileLane<F, N, D, W
     }
 }
 
-// a1-a3, once per tile: doubled prefix sums, invariants, batch-inverted propagators, status.
-// On entry the momenta k_1..k_m are parked in rows [PARK, PARK + m) (see tile_park_row); ends with
-// a block barrier.
+// a1-a3, once per tile: prefix() forms the doubled prefix sums, propagators() the invariants, the
+// batch-inverted propagators and the status word; each ends with a block barrier.  On entry the momenta
+// k_1..k_m are parked in rows [PARK, PARK + m).  singles() (per state configuration) only needs the
+// prefix sums, so the first configuration's runs between the two without a barrier of its own.
 template <class F, int N, int D, int W, int S>
 struct TileSetup {
     typedef TileCfg<F, N, D, W, S> C;
@@ -134,11 +135,9 @@ struct TileSetup {
     static constexpr bool kParPrefix = W > 1 && C::R >= M;
     static constexpr int PARK = kParPrefix ? N : C::PS0 + 1;
 
-    template <int MET>
-    __device__ __forceinline__ static void momenta(const F& f, const TileLane<F, N, D, W, S>& t, uint32_t* status_out)
+    __device__ __forceinline__ static void prefix(const F& f, const TileLane<F, N, D, W, S>& t)
     {
         E* rec = t.rec();
-        E* sc = t.sc();
         // ---- a1: doubled prefix sums PS2_c = 2 (k_1 + .. + k_c)  (Eq.(7)) ------------
         if constexpr (kParPrefix) {
             // row c is formed by warp (c-1) mod W from the parked momenta (same left-to-right order
@@ -178,7 +177,14 @@ struct TileSetup {
             }
         }
         __syncthreads();
+    }
 
+    // a2 + a3 (needs the prefix sums; ends with a block barrier)
+    template <int MET>
+    __device__ __forceinline__ static void propagators(const F& f, const TileLane<F, N, D, W, S>& t,
+                                                       uint32_t* status_out)
+    {
+        E* sc = t.sc();
         // ---- a2 + a3: invariants 4 P_{i,j}^2 and propagators 1/P^2 = 4/(4P^2).  The R proper ranges
         //      are dealt round-robin to the W*S (half-)warps, each lane working on whole vectors here;
         //      every (half-)warp batch-inverts its own share with Montgomery's trick: ONE field

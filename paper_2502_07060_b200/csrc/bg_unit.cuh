@@ -256,7 +256,9 @@ __global__ void __launch_bounds__(32 * W, TileCfg<F, N, D, W, S>::MIN_BLOCKS) bg
     tile_stage<F, N, D, W, S, 0, N>(f, t, gpol, (long long)states * ND, perm);
     __syncthreads();
     // ---- a1-a3: prefix sums, invariants, propagators (momenta only: once per tile and ordering) ----
-    Setup::template momenta<MET>(f, t, gstat);
+    Setup::prefix(f, t);
+    Setup::template singles<MET>(f, t, prm.currents);          // first state configuration
+    Setup::template propagators<MET>(f, t, gstat);
 
 #pragma unroll 1
     for (int s = 0; s < states; ++s) {
@@ -264,9 +266,9 @@ __global__ void __launch_bounds__(32 * W, TileCfg<F, N, D, W, S>::MIN_BLOCKS) bg
             __syncthreads();                                   // the previous sweep is done with eps_n
             tile_stage<F, N, D, W, S, 0, N>(f, t, gpol + (long long)s * ND, (long long)states * ND, perm);
             __syncthreads();
+            Setup::template singles<MET>(f, t, prm.currents);
+            __syncthreads();
         }
-        Setup::template singles<MET>(f, t, prm.currents);
-        __syncthreads();
 
         // ---- a4-a6: level sweep L = 2..m (Eq.(6)), amplitude, store --------------------
 #pragma unroll 1
