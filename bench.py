@@ -378,7 +378,7 @@ def run_features(binding, torch, steps: int) -> list:
     row(f"f4 colour orderings: n=8 d=6 F_p, 2^15 points x K={K}", bo * K,
         time_device(torch, lambda: ev(pb, bo, mom, pol, outk), steps))
     # the general kernel (shapes outside the compiled grid): the performance cliff bg.h documents
-    for (gn, gd, gb) in ((11, 5, 1 << 16), (16, 4, 1 << 14)):
+    for (gn, gd, gb) in ((13, 5, 1 << 15), (16, 4, 1 << 14)):
         mom, pol, _ = B.generate(B.FIELD_FP31, gn, gd, gb, seed=0)
         outg = torch.empty(gb, dtype=torch.int32, device="cuda")
         pb = B.problem(B.FIELD_FP31, gn, gd)

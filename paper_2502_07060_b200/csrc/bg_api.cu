@@ -246,6 +246,19 @@ bool bg_spinor_consts_fp(uint32_t p, int metric, const bg::FpMont::Params* q, ui
 
 namespace {
 
+int sm_count()
+{
+    static std::atomic<int> cached[kMaxDevices];
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) { cudaGetLastError(); return 0; }
+    int n = cached[dev].load(std::memory_order_relaxed);
+    if (n == 0) {
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { cudaGetLastError(); n = 0; }
+        cached[dev].store(n, std::memory_order_relaxed);
+    }
+    return n;
+}
+
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 template <class F>
@@ -268,8 +281,12 @@ int launch_typed(Launch* L, const bg_problem_t& pb, const typename F::Params& fl
     prm.fld = fld;
     int rc = ensure_attr(L);
     if (rc != BG_OK) return rc;
-    const int64_t blocks = (batch + L->points_per_block - 1) / L->points_per_block;
+    int64_t blocks = (batch + L->points_per_block - 1) / L->points_per_block;
     if (blocks > 0x7fffffffLL) return BG_ERR_ARG;
+    if (L->kind == BG_KIND_REG) {                       // persistent warps: at most the resident blocks of the device
+        const int64_t resident = (int64_t)sm_count() * (kSmemPerSm / (L->smem + kSmemReservedPerBlock));
+        if (resident > 0 && blocks > resident) blocks = resident;
+    }
     const unsigned gy = pb.field == BG_FIELD_FPMONT ? (unsigned)pb.n_primes : 1u;
     void* args[] = {&prm};
     if (cudaLaunchKernel(L->func, dim3((unsigned)blocks, gy), dim3(L->threads), args, L->smem, stream) != cudaSuccess) {

@@ -23,7 +23,7 @@ struct KernelEntry {
 };
 
 // first entry of a shape = the default; the others are reachable through bg_set_kernel_override
-#define BG_ENTRY_TABLES(X) X(default) X(fp_alt) X(c128_alt) X(paper) X(grid0) X(grid1) X(grid2) X(cgrid0) X(cgrid1) \
+#define BG_ENTRY_TABLES(X) X(default) X(fp_alt) X(c128_alt) X(paper) X(grid0) X(grid1) X(grid2) X(grid3) X(cgrid0) X(cgrid1) \
     X(metric) X(mont)
 #define BG_DECLARE_TABLE(name) const KernelEntry* bg_entries_##name(int* count);
 BG_ENTRY_TABLES(BG_DECLARE_TABLE)

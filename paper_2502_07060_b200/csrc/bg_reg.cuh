@@ -15,6 +15,8 @@
 // of the two lanes' partial products (bg_split.cuh).  Inputs are read straight from global memory
 // into registers (32 contiguous bytes per lane and row).
 #pragma once
+#include <cuda_pipeline.h>
+
 #include "bg_common.cuh"
 #include "bg_schedule.cuh"
 
@@ -32,7 +34,11 @@ struct RegCfg {
     static constexpr int NSCAL = W_OFF + R;
     static constexpr int WARPS = 4;                           // independent warps per block
     static constexpr int MIN_BLOCKS = 2;                      // 236 registers, no spills (3 blocks: 168 registers, 80 B of spills, same speed)
-    static constexpr size_t SMEM_BYTES = (size_t)WARPS * NSCAL * TP * sizeof(E);
+    // input staging buffer of a warp: eps_1..eps_n and k_1..k_m of its NEXT 16 points, copied with cp.async
+    // while the current 16 points are computed; point stride an odd number of elements (conflict-free)
+    static constexpr int IN_ROWS = N + M;
+    static constexpr int IN_STRIDE = (IN_ROWS * D) | 1;
+    static constexpr size_t SMEM_BYTES = (size_t)WARPS * (NSCAL + IN_STRIDE) * TP * sizeof(E);
 };
 
 // row of J(i..i+len-1), i 1-based
@@ -66,40 +72,68 @@ __global__ void __launch_bounds__(32 * RegCfg<F, N, D>::WARPS, RegCfg<F, N, D>::
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int point = lane & (TP - 1), half = lane / TP, mu0 = half * DL;
     const F f(prm.fld, 0);
-    E* sc = reinterpret_cast<E*>(smem_raw) + (size_t)warp * C::NSCAL * TP + point;   // [index][TP], this point's column
-    const long long pt = ((long long)blockIdx.x * C::WARPS + warp) * TP + point;
+    E* wbase = reinterpret_cast<E*>(smem_raw) + (size_t)warp * (C::NSCAL + C::IN_STRIDE) * TP;
+    E* sc = wbase + point;                                    // [index][TP], this point's column
+    E* inbuf = wbase + C::NSCAL * TP;                         // [TP][IN_STRIDE]
+    // Persistent warps: warp w of the grid owns the 16-point groups w, w + (warps in the grid), ...  The inputs
+    // of the next group are copied global -> shared with cp.async while the current group is computed, so the
+    // HBM latency (17 % of the stall samples when the inputs went straight to registers) is off the critical path.
+    const long long ngroups = (prm.batch + TP - 1) / TP;
+    const long long gstep = (long long)gridDim.x * C::WARPS;
+    auto prefetch = [&](long long g) {
+        constexpr int CH_POL = N * D, CH = C::IN_ROWS * D;    // elements per point: eps rows, then k_1..k_m
+        for (int idx = lane; idx < TP * CH; idx += 32) {
+            const int p = idx / CH, w = idx - p * CH;
+            long long gp = g * TP + p;
+            gp = gp < prm.batch ? gp : prm.batch - 1;         // ragged last group: repeat the last point (no stores)
+            const E* src = w < CH_POL ? prm.pol + gp * ND + w : prm.mom + gp * ND + (w - CH_POL);
+            __pipeline_memcpy_async(inbuf + p * C::IN_STRIDE + w, src, sizeof(E));
+        }
+        __pipeline_commit();
+    };
+    long long g = (long long)blockIdx.x * C::WARPS + warp;
+    if (g < ngroups) prefetch(g);
+#pragma unroll 1
+    for (; g < ngroups; g += gstep) {
+    const long long pt = g * TP + point;
     const bool live = pt < prm.batch;
-    const long long ptc = live ? pt : prm.batch - 1;          // dead lanes recompute the last point (no stores)
 
     E J[C::J_ROWS + 1][DL];                                   // + the top current
     uint32_t status = 0;
 
     // ---- a0/a1: eps rows into registers; doubled prefix sums PS2_c into the lane's column; U = V = 2 k.eps
+    __pipeline_wait_prior(0);
+    __syncwarp();
     {
-        const E* gp = prm.pol + ptc * ND + half * DL;
-        const E* gm = prm.mom + ptc * ND + half * DL;
+        const E* gp = inbuf + point * C::IN_STRIDE + half * DL;
+        const E* gm = gp + N * D;
         E run[DL];
 #pragma unroll
         for (int mu = 0; mu < DL; ++mu) {
             run[mu] = f.ezero();
             sc[(C::PS_OFF + mu + half * DL) * TP] = run[mu];
         }
+        E kk[M][DL];
 #pragma unroll
         for (int c = 1; c <= N; ++c) {
 #pragma unroll
-            for (int mu = 0; mu < DL; ++mu) J[c - 1][mu] = f.load_input(__ldg(gp + (c - 1) * D + mu));
+            for (int mu = 0; mu < DL; ++mu) J[c - 1][mu] = f.load_input(gp[(c - 1) * D + mu]);
             if (c <= M) {
-                E k[DL];
 #pragma unroll
-                for (int mu = 0; mu < DL; ++mu) k[mu] = f.dbl(f.load_input(__ldg(gm + (c - 1) * D + mu)));
-                const E u = f.neg(reg_dot_neg<F, MET, DL, TP>(f, mu0, k, J[c - 1]));       // 2 k.eps
-                sc[(C::U_OFF + c - 1) * TP] = u;
-                sc[(C::V_OFF + c - 1) * TP] = u;
+                for (int mu = 0; mu < DL; ++mu) kk[c - 1][mu] = f.dbl(f.load_input(gm[(c - 1) * D + mu]));
+            }
+        }
+        __syncwarp();                                          // every lane has its inputs: the buffer is free
+        if (g + gstep < ngroups) prefetch(g + gstep);
 #pragma unroll
-                for (int mu = 0; mu < DL; ++mu) {
-                    run[mu] = f.add(run[mu], k[mu]);
-                    sc[(C::PS_OFF + c * D + mu + half * DL) * TP] = run[mu];
-                }
+        for (int c = 1; c <= M; ++c) {
+            const E u = f.neg(reg_dot_neg<F, MET, DL, TP>(f, mu0, kk[c - 1], J[c - 1]));       // 2 k.eps
+            sc[(C::U_OFF + c - 1) * TP] = u;
+            sc[(C::V_OFF + c - 1) * TP] = u;
+#pragma unroll
+            for (int mu = 0; mu < DL; ++mu) {
+                run[mu] = f.add(run[mu], kk[c - 1][mu]);
+                sc[(C::PS_OFF + c * D + mu + half * DL) * TP] = run[mu];
             }
         }
     }
@@ -205,6 +239,8 @@ __global__ void __launch_bounds__(32 * RegCfg<F, N, D>::WARPS, RegCfg<F, N, D>::
         }
     }
     if (prm.status && live && half == 0) prm.status[pt] = status;
+    __syncwarp();                                              // lane-private columns are rewritten by the next group
+    }
 }
 
 }  // namespace bg

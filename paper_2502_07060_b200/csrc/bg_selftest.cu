@@ -96,5 +96,6 @@ extern "C" int bg_selftest_schedules(void)
     if ((rc = check_level_program<12, 16>())) return rc - 160000;
     if ((rc = check_level_program<12, 4>())) return rc - 170000;
     if ((rc = check_level_program<16, 8>())) return rc - 180000;
+    if ((rc = check_level_program<11, 8>())) return rc - 190000;
     return rc;
 }

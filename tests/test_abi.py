@@ -62,7 +62,7 @@ def test_kernel_info_and_bad_shapes(lib):
     ki = binding.bg_kernel_info(0, 8, 6)
     assert ki["specialised"] >= 1 and ki["points_per_block"] in (16, 32) and ki["threads_per_block"] % 32 == 0
     assert ki["smem_bytes_per_block"] <= 232448
-    assert binding.bg_kernel_info(0, 11, 5)["specialised"] == 0      # outside the compiled grid: general kernel
+    assert binding.bg_kernel_info(0, 13, 5)["specialised"] == 0      # outside the compiled grid: general kernel
     assert binding.bg_kernel_info(1, 6, 4)["specialised"] == 3       # cfg1: bg_reg_kernel ...
     pb = binding.problem(1, 6, 4, states=4)
     assert binding.bg_kernel_info_problem(pb)["specialised"] == 2    # ... but not with several state configurations

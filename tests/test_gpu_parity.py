@@ -69,7 +69,8 @@ def _assert_rule(mom, pol, got, tag=None):
 
 # sizes span several 32-point tiles and a ragged tail
 FP_SHAPES = [(4, 4, 1024), (8, 6, 517), (10, 8, 197), (12, 6, 133),     # the config shapes
-             (5, 5, 99), (6, 4, 200), (7, 5, 77), (9, 7, 45), (5, 16, 40), (16, 4, 37), (13, 9, 35)]
+             (5, 5, 99), (6, 4, 200), (7, 5, 77), (9, 7, 45), (5, 16, 40), (16, 4, 37), (13, 9, 35),
+             (11, 4, 70), (11, 5, 45), (11, 6, 70), (11, 8, 40), (12, 4, 70), (12, 5, 45), (12, 8, 40)]
 
 
 @pytest.mark.parametrize("n,d,batch", FP_SHAPES, ids=lambda v: str(v))
