@@ -199,10 +199,81 @@ __device__ __forceinline__ void unit_finish(const F& f, const TileLane<F, N, D, 
     }
 }
 
+// a4-a6 for one state configuration of one tile: the level sweep L = 2..m (Eq.(6)), amplitude, store.
+template <class F, int MET, int N, int D, int W, int S>
+__device__ __forceinline__ void unit_sweep_body(const F& f, const TileLane<F, N, D, W, S>& t, const int warp,
+                                                typename F::E* out, typename F::E* currents)
+{
+    typedef TileCfg<F, N, D, W, S> C;
+    typedef typename F::E E;
+    typedef typename F::A A;
+    constexpr int M = N - 1, DL = C::DL, TP = C::TP;
+    const LevelProgram<N, W>& tb = c_level_program<F, N, D, W>;
+    const UnitTable<N>& ut = c_unit_table<F, N, D, W, S>;
+    E* rec = t.rec();
+    E* sc = t.sc();
+    // ---- a4-a6: level sweep L = 2..m (Eq.(6)), amplitude, store --------------------
+#pragma unroll 1
+    for (int L = 2; L <= M; ++L) {
+        const int lbase = UnitTable<N>::index(L, 1);
+        const int own = ut.u[lbase].own, widx = ut.u[lbase].w;
+        const int t0 = tb.beg[L][warp], t1 = tb.beg[L][warp + 1];
+#pragma unroll 1
+        for (int k = t0; k < t1; ++k) {
+            const uint32_t ta = tb.task[k].a;
+            if (ta & LT_BAR) __syncthreads();
+            if (!(ta & (LT_FIN | LT_PART))) continue;
+            const int ci = ta & 15u, lo = ta >> 4 & 15u, hi = ta >> 8 & 15u;
+            E* ri = rec + ci * D;
+            E* si = sc + ci * TP;
+            E l[DL], h[DL], x2[DL];
+            ld_vec<F, DL>(ri + C::PS0 * D, l);                     // PS2_{i-1}
+            ld_vec<F, DL>(ri + (C::PS0 + L) * D, h);               // PS2_j
+            lower_diff<F, MET, DL>(f, t.mu0, h, l, x2);            // 2 * covariant P_{i,j}
+            A acc[DL];
+#pragma unroll
+            for (int mu = 0; mu < DL; ++mu) acc[mu] = f.zero();
+            E hsum = f.ezero();
+#pragma unroll 1
+            for (int la = lo + 1; la <= hi; ++la)
+                UnitDispatch<F, MET, N, D, S, N - 3>::run(f, t.mu0, L - la - 1, ri, si, ut.u[lbase + la - 1], x2,
+                                                          acc, hsum);
+            uint32_t mask = tb.task[k].mask;
+            if (mask) {                                            // gather task (no units of its own)
+                E sum[DL];
+#pragma unroll
+                for (int mu = 0; mu < DL; ++mu) sum[mu] = f.ezero();
+                while (mask) {
+                    const int slot = __ffs(mask) - 1;
+                    mask &= mask - 1;
+                    const E* scr = sc + (C::SC_SCR + slot * (D + 1)) * TP;
+#pragma unroll
+                    for (int mu = 0; mu < DL; ++mu) sum[mu] = f.add(sum[mu], scr[(t.mu0 + mu) * TP]);
+                    hsum = f.add(hsum, scr[D * TP]);
+                }
+#pragma unroll
+                for (int mu = 0; mu < DL; ++mu) acc[mu] = f.widen(sum[mu]);
+            }
+            if (ta & LT_PART) {
+                E* scr = sc + (C::SC_SCR + (ta >> 12 & 63u) * (D + 1)) * TP;
+#pragma unroll
+                for (int mu = 0; mu < DL; ++mu) scr[(t.mu0 + mu) * TP] = f.reduce(acc[mu]);
+                scr[D * TP] = hsum;
+                continue;
+            }
+            unit_finish<F, MET, N, D, W, S>(f, t, ri, si, l, h, x2, acc, hsum, ci, L, own, widx, out,
+                                            currents);
+        }
+        if (L < M) __syncthreads();
+    }
+}
+
 // MULTI = false: one state configuration and one colour ordering per point, no loops around the sweep (the
 // headline path).  MULTI = true adds the loops over orderings and state configurations; it is a separate
 // instantiation because ptxas stops using the uniform datapath for the control flow and the table loads of
-// the sweep once it sits inside another loop (+12 % executed instructions, measured on cfg3).
+// the sweep once it sits inside another loop (+12 % executed instructions, measured on cfg3).  (Calling the sweep
+// as a __noinline__ function from the loops brings part of the uniform code back but costs more than it saves:
+// S = 4 at cfg2's shape 1.00 -> 1.15 ms.)
 template <class F, int MET, int N, int D, int W, int S, bool MULTI>
 __global__ void __launch_bounds__(32 * W, TileCfg<F, N, D, W, S>::MIN_BLOCKS) bg_unit_kernel(const BgParams<F> prm)
 {
@@ -270,60 +341,7 @@ __global__ void __launch_bounds__(32 * W, TileCfg<F, N, D, W, S>::MIN_BLOCKS) bg
             __syncthreads();
         }
 
-        // ---- a4-a6: level sweep L = 2..m (Eq.(6)), amplitude, store --------------------
-#pragma unroll 1
-        for (int L = 2; L <= M; ++L) {
-            const int lbase = UnitTable<N>::index(L, 1);
-            const int own = ut.u[lbase].own, widx = ut.u[lbase].w;
-            const int t0 = tb.beg[L][warp], t1 = tb.beg[L][warp + 1];
-#pragma unroll 1
-            for (int k = t0; k < t1; ++k) {
-                const uint32_t ta = tb.task[k].a;
-                if (ta & LT_BAR) __syncthreads();
-                if (!(ta & (LT_FIN | LT_PART))) continue;
-                const int ci = ta & 15u, lo = ta >> 4 & 15u, hi = ta >> 8 & 15u;
-                E* ri = rec + ci * D;
-                E* si = sc + ci * TP;
-                E l[DL], h[DL], x2[DL];
-                ld_vec<F, DL>(ri + C::PS0 * D, l);                     // PS2_{i-1}
-                ld_vec<F, DL>(ri + (C::PS0 + L) * D, h);               // PS2_j
-                lower_diff<F, MET, DL>(f, t.mu0, h, l, x2);            // 2 * covariant P_{i,j}
-                A acc[DL];
-#pragma unroll
-                for (int mu = 0; mu < DL; ++mu) acc[mu] = f.zero();
-                E hsum = f.ezero();
-#pragma unroll 1
-                for (int la = lo + 1; la <= hi; ++la)
-                    UnitDispatch<F, MET, N, D, S, N - 3>::run(f, t.mu0, L - la - 1, ri, si, ut.u[lbase + la - 1], x2,
-                                                              acc, hsum);
-                uint32_t mask = tb.task[k].mask;
-                if (mask) {                                            // gather task (no units of its own)
-                    E sum[DL];
-#pragma unroll
-                    for (int mu = 0; mu < DL; ++mu) sum[mu] = f.ezero();
-                    while (mask) {
-                        const int slot = __ffs(mask) - 1;
-                        mask &= mask - 1;
-                        const E* scr = sc + (C::SC_SCR + slot * (D + 1)) * TP;
-#pragma unroll
-                        for (int mu = 0; mu < DL; ++mu) sum[mu] = f.add(sum[mu], scr[(t.mu0 + mu) * TP]);
-                        hsum = f.add(hsum, scr[D * TP]);
-                    }
-#pragma unroll
-                    for (int mu = 0; mu < DL; ++mu) acc[mu] = f.widen(sum[mu]);
-                }
-                if (ta & LT_PART) {
-                    E* scr = sc + (C::SC_SCR + (ta >> 12 & 63u) * (D + 1)) * TP;
-#pragma unroll
-                    for (int mu = 0; mu < DL; ++mu) scr[(t.mu0 + mu) * TP] = f.reduce(acc[mu]);
-                    scr[D * TP] = hsum;
-                    continue;
-                }
-                unit_finish<F, MET, N, D, W, S>(f, t, ri, si, l, h, x2, acc, hsum, ci, L, own, widx, gout + s,
-                                                prm.currents);
-            }
-            if (L < M) __syncthreads();
-        }
+        unit_sweep_body<F, MET, N, D, W, S>(f, t, warp, gout + s, prm.currents);
     }
     }
 }
