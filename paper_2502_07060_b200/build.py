@@ -22,6 +22,8 @@ HEADERS = ["bg_field.cuh", "bg_common.cuh", "bg_schedule.cuh", "bg_tile.cuh", "b
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-Xcompiler", "-fPIC", "-Xptxas", "-v", "-Xptxas", "-warn-spills",
+    # the schedules (bg_schedule.cuh) are found by constexpr dynamic programming, also in the host pass
+    "-Xcompiler", "-fconstexpr-ops-limit=2000000000",
 ]
 
 

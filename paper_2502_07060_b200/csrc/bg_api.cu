@@ -75,7 +75,7 @@ const KernelEntry* find_entry(int field, int metric, int n, int d, bool multi_st
         for (int i = 0; i < count; ++i) {
             const KernelEntry& e = t[i];
             if (e.field != field || e.metric != metric || e.n != n || e.d != d) continue;
-            if (e.smem > (size_t)kMaxSmemPerBlock) continue;
+            if ((multi_state ? e.smem_multi : e.smem) > (size_t)kMaxSmemPerBlock) continue;
             if (multi_state && !e.func_multi) continue;                 // bg_reg_kernel: one configuration only
             if (want_kind >= 0 && e.kind != want_kind) continue;
             if (!first) first = &e;
@@ -118,7 +118,7 @@ void fill_entry(const KernelEntry& e, bool multi, Launch* L)
     L->kind = e.kind;
     L->threads = 32 * e.w;
     L->points_per_block = e.tp;
-    L->smem = (int)e.smem;
+    L->smem = (int)(multi ? e.smem_multi : e.smem);
     L->stride = 0;
 }
 

@@ -19,7 +19,8 @@ struct KernelEntry {
     int tp;                  // points per block
     const void* func;        // one state configuration, one ordering
     const void* func_multi;  // loops over orderings and state configurations; NULL: not available (bg_reg_kernel)
-    size_t smem;
+    size_t smem;             // dynamic shared memory of func
+    size_t smem_multi;       // ... of func_multi (keeps the propagators in a table of their own)
 };
 
 // first entry of a shape = the default; the others are reachable through bg_set_kernel_override

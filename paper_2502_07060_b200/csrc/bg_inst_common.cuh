@@ -19,14 +19,14 @@ KernelEntry unit_entry()
     return KernelEntry{F::kFieldId, MET, N, D, W, S == 1 ? BG_KIND_UNIT1 : BG_KIND_UNIT2, 32 / S,
                        reinterpret_cast<const void*>(&bg::bg_unit_kernel<F, MET, N, D, W, S, false>),
                        reinterpret_cast<const void*>(&bg::bg_unit_kernel<F, MET, N, D, W, S, true>),
-                       bg::TileCfg<F, N, D, W, S>::SMEM_BYTES};
+                       bg::TileCfg<F, N, D, W, S, false>::SMEM_BYTES, bg::TileCfg<F, N, D, W, S, true>::SMEM_BYTES};
 }
 template <class F, int MET, int N, int D>
 KernelEntry reg_entry()
 {
     return KernelEntry{F::kFieldId, MET, N, D, bg::RegCfg<F, N, D>::WARPS, BG_KIND_REG, 16 * bg::RegCfg<F, N, D>::WARPS,
                        reinterpret_cast<const void*>(&bg::bg_reg_kernel<F, MET, N, D>), nullptr,
-                       bg::RegCfg<F, N, D>::SMEM_BYTES};
+                       bg::RegCfg<F, N, D>::SMEM_BYTES, 0};
 }
 
 }  // namespace

@@ -40,7 +40,10 @@ struct LevelTask {
 struct LevelWeights {
     int w3, w4, wstart, wfin, wpart, wgather;
 };
-constexpr LevelWeights kLevelWeights = {95, 30, 50, 125, 60, 30};   // from the ncu source view, profiles/r01b
+#ifndef BG_LEVEL_WEIGHTS
+#define BG_LEVEL_WEIGHTS {95, 30, 50, 125, 60, 30}   // from the ncu source view, profiles/r01b
+#endif
+constexpr LevelWeights kLevelWeights = BG_LEVEL_WEIGHTS;
 
 template <int N, int W>
 struct LevelProgram {
@@ -48,6 +51,7 @@ struct LevelProgram {
     static constexpr int MAXT = M * (M + 1) / 2 + 4 * W * M;
     LevelTask task[MAXT];
     uint16_t beg[M + 1][W + 1];          // tasks of warp w at level L: [beg[L][w], beg[L][w+1])
+    int nslots;                          // scratch slots in use at once (slots are numbered per level)
 };
 
 template <int N, int W>
@@ -130,6 +134,7 @@ constexpr LevelProgram<N, W> make_level_program(LevelWeights wt = kLevelWeights)
         LevelTask tmp[W][PER] = {};
         int ntw[W] = {};
         long load[W] = {};
+        int nslot = 0;
         // phase A tasks
         for (int w = 0; w < W; ++w) {
             const int ub = cut[w], ue = cut[w + 1];
@@ -138,7 +143,7 @@ constexpr LevelProgram<N, W> make_level_program(LevelWeights wt = kLevelWeights)
                 const int lo = ub - ci * NU > 0 ? ub - ci * NU : 0;
                 const int hi = ue - ci * NU < NU ? ue - ci * NU : NU;
                 const bool complete = lo == 0 && hi == NU;
-                const int slot = 2 * w + (lo > 0 ? 0 : 1);
+                const int slot = complete ? 0 : nslot++;
                 tmp[w][ntw[w]].a = (uint32_t)ci | (uint32_t)lo << 4 | (uint32_t)hi << 8 |
                                    (complete ? LT_FIN : ((uint32_t)slot << 12 | LT_PART));
                 tmp[w][ntw[w]].mask = 0;
@@ -180,9 +185,16 @@ constexpr LevelProgram<N, W> make_level_program(LevelWeights wt = kLevelWeights)
             for (int t = 0; t < ntw[w] + nb[w]; ++t) p.task[nt++] = tmp[w][t];
         }
         p.beg[L][W] = (uint16_t)nt;
+        if (nslot > p.nslots) p.nslots = nslot;
     }
     return p;
 }
+
+// the schedule of (n, warps), evaluated once per instantiation
+template <int N, int W>
+struct LevelProgramOf {
+    static constexpr LevelProgram<N, W> value = make_level_program<N, W>();
+};
 
 // row of J(1..la) in the vector record; J(i..i+la-1) is row lv_rowbase(la) + (i-1)
 template <int N>

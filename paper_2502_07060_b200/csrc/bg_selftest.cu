@@ -43,7 +43,7 @@ int check_level_program()
                 for (int u = lo; u < hi; ++u) ++covered[ci][u];
                 if (a & LT_PART) {
                     if (seen_bar || mask || lo == hi) return -400 - L;    // parts come before the barrier
-                    if (slot >= 2 * W || (level_slots >> slot & 1u)) return -500 - L;
+                    if (slot >= p.nslots || (level_slots >> slot & 1u)) return -500 - L;
                     level_slots |= 1u << slot;
                     part_slots[ci] |= 1u << slot;
                     ++parts[ci];

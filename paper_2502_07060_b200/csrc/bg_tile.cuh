@@ -13,9 +13,9 @@
 //                   rows [n, n+R)     multi-gluon currents J(i..j), level-major, top excluded
 //                   rows PS0 + c      doubled prefix sums PS2_c = 2 (k_1+..+k_c), c = 0..m
 //                                     (Eq.(7))
-//   scalar tables:  U, V per row      U = 2 P.J + S,  V = 2 P.J - S   (P own momentum)
-//                   Wt per proper multi-gluon range: 1/P^2 (batch-inverted)
-//                   scratch           partial sums of currents shared between warps, 2 slots per warp
+//   scalar tables:  U, V per row      U = 2 P.J + S,  V = 2 P.J - S   (P own momentum; V = U for single gluons)
+//                   1/P^2 per proper multi-gluon range (batch-inverted), parked in the range's U slot
+//                   scratch           partial sums of currents shared between warps
 //
 // PS2, Wt and the status word depend on the momenta only: with S_c > 1 state configurations per
 // momentum point (Eq.(4): "the state sum runs over all D_s-dimensional particle
@@ -26,7 +26,7 @@
 
 namespace bg {
 
-template <class F, int N, int D, int W, int S>
+template <class F, int N, int D, int W, int S, bool KW>
 struct TileCfg {
     typedef typename F::E E;
     static_assert(S == 1 || S == 2, "one or two lanes per point");
@@ -41,8 +41,13 @@ struct TileCfg {
     static constexpr int VEC_ROWS = J_ROWS + M + 1;
     static constexpr int VEC_ELEMS = VEC_ROWS * D;
     static constexpr int VSTRIDE = (VEC_ELEMS / U % 2 == 1 ? VEC_ELEMS / U : VEC_ELEMS / U + 1) * U;
-    static constexpr int SC_U = 0, SC_V = J_ROWS, SC_W = 2 * J_ROWS, SC_SCR = 2 * J_ROWS + R;
-    static constexpr int NSLOTS = 2 * W;
+    // scalar tables [index][point]: U per row; V per multi-gluon row (the single-gluon rows have V = U);
+    // 1/P^2 of a proper range lives in the U slot of its current until the current is finished (the finish
+    // reads it, then writes U); scratch slots for the partial sums of currents shared between warps
+    // (KW: a table of its own instead -- with several state configurations per point the propagators outlive a sweep)
+    static constexpr int SC_U = 0, SC_V = J_ROWS, SC_W = KW ? J_ROWS + R : SC_U + N, SC_SCR = J_ROWS + R + (KW ? R : 0);
+    __host__ __device__ static constexpr int v_index(int row) { return row < N ? SC_U + row : SC_V + row - N; }
+    static constexpr int NSLOTS = LevelProgramOf<N, W>::value.nslots;
     static constexpr int NSCAL = SC_SCR + NSLOTS * (D + 1);
     static constexpr int THREADS = 32 * W;
     static constexpr size_t SMEM_BYTES = (size_t)TP * (VSTRIDE + NSCAL) * sizeof(E) + TP * sizeof(uint32_t);
@@ -72,9 +77,9 @@ template <int N>
 __constant__ TileRanges<N> c_tile_ranges = make_tile_ranges<N>();
 
 // the lane's view of its tile
-template <class F, int N, int D, int W, int S>
+template <class F, int N, int D, int W, int S, bool KW>
 struct TileLane {
-    typedef TileCfg<F, N, D, W, S> C;
+    typedef TileCfg<F, N, D, W, S, KW> C;
     typedef typename F::E E;
     E* vec;               // [TP][VSTRIDE]
     E* scal;              // [NSCAL][TP]
@@ -92,22 +97,55 @@ struct TileLane {
 // step).  src: first element of point tile0's block; a point's block is ND elements, consecutive
 // points are `pstride` elements apart; the first ROWS rows go to record rows [ROW0, ROW0 + ROWS).
 // perm: NULL, or the colour ordering (Eq.(5)): record row ROW0 + i receives the caller's row perm[i].
-template <class F, int N, int D, int W, int S, int ROW0, int ROWS>
-__device__ __forceinline__ void tile_stage(const F& f, const TileLane<F, N, D, W, S>& t, const typename F::E* src,
+template <class F, int N, int D, int W, int S, bool KW, int ROW0, int ROWS>
+__device__ __forceinline__ void tile_stage(const F& f, const TileLane<F, N, D, W, S, KW>& t, const typename F::E* src,
                                            long long pstride, const unsigned char* __restrict__ perm)
 {
-    typedef TileCfg<F, N, D, W, S> C;
+    typedef TileCfg<F, N, D, W, S, KW> C;
     typedef typename VecType<F, C::U>::type V;
     constexpr int U = C::U, row0 = ROW0;
     constexpr int upp = ROWS * D / U;                           // units per point
     constexpr int upr = D / U;                                  // units per row
     const int total = t.valid * upp;
     if (perm == nullptr) {
-#pragma unroll 4
-        for (int g = threadIdx.x; g < total; g += 32 * W) {
-            const int p = g / upp, u = g - p * upp;
-            V* r = reinterpret_cast<V*>(t.vec + (size_t)p * C::VSTRIDE) + row0 * D / U;
-            r[u] = load_unit<F>(f, __ldg(reinterpret_cast<const V*>(src + p * pstride) + u));
+        // Thread tid moves the units g = tid + j THREADS, j = 0..NIT-1.  (point, unit-in-point) and both
+        // addresses advance incrementally (no division, no 64-bit multiply per unit), and ALL loads of
+        // a thread are issued before the first store: one global-memory latency per stage instead of
+        // one per batch of four (the staging loops were 9 % of the instructions and the
+        // long-scoreboard stall of the round-2 profile).
+        constexpr int T = 32 * W;
+        constexpr int NIT = (C::TP * upp + T - 1) / T;
+        constexpr int dp = T / upp, du = T % upp;               // advance of (point, unit) per step
+        constexpr int VS = C::VSTRIDE / U;                      // record stride in units
+        const int ps = (int)(pstride / U);                      // source stride in units
+        const int p0 = threadIdx.x / upp, u0 = threadIdx.x - p0 * upp;
+        constexpr int CHUNK = 24 / (int)(sizeof(V) / 4) > 0 ? 24 / (int)(sizeof(V) / 4) : 1;   // <= 24 registers in flight
+        const V* s = reinterpret_cast<const V*>(src) + (long long)p0 * ps + u0;
+        V* r = reinterpret_cast<V*>(t.vec) + p0 * VS + row0 * D / U + u0;
+        int us = u0, ur = u0, gs = threadIdx.x, gr = threadIdx.x;
+#pragma unroll
+        for (int j0 = 0; j0 < NIT; j0 += CHUNK) {
+            V buf[CHUNK];
+#pragma unroll
+            for (int j = 0; j < CHUNK; ++j) {
+                if (j0 + j < NIT) {
+                    if (gs < total) buf[j] = __ldg(s);
+                    gs += T;
+                    us += du;
+                    s += dp * ps + du;
+                    if (du != 0 && us >= upp) { us -= upp; s += ps - upp; }
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < CHUNK; ++j) {
+                if (j0 + j < NIT) {
+                    if (gr < total) *r = load_unit<F>(f, buf[j]);
+                    gr += T;
+                    ur += du;
+                    r += dp * VS + du;
+                    if (du != 0 && ur >= upp) { ur -= upp; r += VS - upp; }
+                }
+            }
         }
     } else {
 #pragma unroll 2
@@ -123,9 +161,9 @@ __device__ __forceinline__ void tile_stage(const F& f, const TileLane<F, N, D, W
 // batch-inverted propagators and the status word; each ends with a block barrier.  On entry the momenta
 // k_1..k_m are parked in rows [PARK, PARK + m).  singles() (per state configuration) only needs the
 // prefix sums, so the first configuration's runs between the two without a barrier of its own.
-template <class F, int N, int D, int W, int S>
+template <class F, int N, int D, int W, int S, bool KW>
 struct TileSetup {
-    typedef TileCfg<F, N, D, W, S> C;
+    typedef TileCfg<F, N, D, W, S, KW> C;
     typedef typename F::E E;
     typedef typename F::A A;
     static constexpr int M = C::M, DL = C::DL, TP = C::TP;
@@ -135,7 +173,7 @@ struct TileSetup {
     static constexpr bool kParPrefix = W > 1 && C::R >= M;
     static constexpr int PARK = kParPrefix ? N : C::PS0 + 1;
 
-    __device__ __forceinline__ static void prefix(const F& f, const TileLane<F, N, D, W, S>& t)
+    __device__ __forceinline__ static void prefix(const F& f, const TileLane<F, N, D, W, S, KW>& t)
     {
         E* rec = t.rec();
         // ---- a1: doubled prefix sums PS2_c = 2 (k_1 + .. + k_c)  (Eq.(7)) ------------
@@ -181,7 +219,7 @@ struct TileSetup {
 
     // a2 + a3 (needs the prefix sums; ends with a block barrier)
     template <int MET>
-    __device__ __forceinline__ static void propagators(const F& f, const TileLane<F, N, D, W, S>& t,
+    __device__ __forceinline__ static void propagators(const F& f, const TileLane<F, N, D, W, S, KW>& t,
                                                        uint32_t* status_out)
     {
         E* sc = t.sc();
@@ -208,9 +246,9 @@ struct TileSetup {
                 Wt[r * TP] = f.canon(f.neg(f.reduce(ns)));
             }
             if constexpr (F::kExact) {
-                // zero-safe (inv(0) := 0, bg.h); prefix products parked in the not-yet-used U slots
+                // zero-safe (inv(0) := 0, bg.h); prefix products parked in the not-yet-used V slots
                 // of the multi-gluon currents
-                E* tmp = sc + (C::SC_U + N) * TP;
+                E* tmp = sc + C::SC_V * TP;
                 E c = f.one();
 #pragma unroll 1
                 for (int r = vw; r < C::R; r += VW) {
@@ -248,7 +286,7 @@ struct TileSetup {
     // per state configuration: the single-gluon U = V = 2 k_c . eps_c (zero for transverse states;
     // kept for any input, R4), 2 k_c = PS2_c - PS2_{c-1}.  No barrier inside.
     template <int MET>
-    __device__ __forceinline__ static void singles(const F& f, const TileLane<F, N, D, W, S>& t,
+    __device__ __forceinline__ static void singles(const F& f, const TileLane<F, N, D, W, S, KW>& t,
                                                    typename F::E* currents)
     {
         E* rec = t.rec();
@@ -262,7 +300,6 @@ struct TileSetup {
             lower_diff<F, MET, DL>(f, t.mu0, hi, lo, k2);                       // 2 * covariant k_c
             const E u = lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, k2, e)));   // 2 k.eps
             sc[(C::SC_U + c - 1) * TP] = u;
-            sc[(C::SC_V + c - 1) * TP] = u;
             if (currents && t.live) {
                 E* dst = currents + (t.pt * M * M + (long long)(c - 1) * M + (c - 1)) * D + t.mu0;
 #pragma unroll

@@ -17,72 +17,156 @@
 
 namespace bg {
 
-template <class F, int N, int D, int W>
-__constant__ LevelProgram<N, W> c_level_program = make_level_program<N, W>();
+// ---- the flat per-warp program ---------------------------------------------------------------------
+// The task lists of bg_schedule.cuh (levels -> tasks -> units) are flattened at compile time into ONE list
+// of ops per warp; an op is one unit (or a gather / a bare barrier) with every operand offset resolved to a
+// byte offset from the lane's record / scalar base, so the sweep is a single run-time loop whose body needs
+// two 16-byte constant loads and a few warp-uniform flag tests (round 2 decoded a task word, a unit-table
+// entry and a level header per iteration: 4.2 k of the 20.3 k instructions per cfg2 tile).
+constexpr uint32_t OP_BAR = 1u;       // block barrier before the op (first gather op of the level)
+constexpr uint32_t OP_START = 2u;     // first op of a task: form 2 P_{i,j}, clear the bracket sums
+constexpr uint32_t OP_UNIT = 4u;      // a 3-gluon split with its c4 4-gluon splits
+constexpr uint32_t OP_PART = 8u;      // last op of a task that owns part of a current: park the partial sums
+constexpr uint32_t OP_FIN = 16u;      // last op of a task: finish the current
+constexpr uint32_t OP_GATHER = 32u;   // sum the parked partial sums (aux = mask of scratch slots)
+constexpr uint32_t OP_LEND = 64u;     // block barrier after the op (end of the level)
+constexpr uint32_t OP_TOP = 128u;     // the current is J(1..m): amplitude instead of propagator and store
 
-// BYTE offsets of the operands of unit (L, la), relative to the current's base pointers
-// ri = rec + ci*D (vector rows) and si = sc + ci*TP (scalar tables): ready for [register + uniform
-// register + immediate] addressing, no per-lane address arithmetic
-template <int N>
-struct UnitOff {
-    static constexpr int MAXC4 = N - 3;                        // c4 = L-la-1 <= M-2
-    uint32_t u, v, w;                                          // scalar tables (w: 1/P^2 of the level's currents)
-    uint16_t a, b, ps;
-    uint16_t own;                                              // per level (same for every la): row of J(i..j)
-    uint16_t bm[MAXC4 > 0 ? MAXC4 : 1], c[MAXC4 > 0 ? MAXC4 : 1];
+struct FlatOp {
+    uint32_t ab;       // row A | row B << 16      (byte offsets in the lane's vector record)
+    uint32_t pso;      // row PS2_k | own row << 16
+    uint32_t u, v;     // U_A, V_B                 (byte offsets from the lane's scalar base)
+    uint32_t w;        // ci * m + j - 1 (position of the current in the caller's `currents` array) | own row << 16
+    uint32_t lh;       // rows PS2_{i-1} | PS2_j << 16
+    uint32_t qcf;      // first entry of the op's 4-gluon splits in quad[] | c4 << 16 | flags << 24
+    uint32_t aux;      // OP_PART: scratch slot (byte offset from the first slot) ; OP_GATHER: mask of slots
 };
 
-template <int N>
-struct UnitTable {
-    // units packed level-major: (L, la), 2 <= L <= N-1, 1 <= la <= L-1, at index (L-1)(L-2)/2 + la-1
-    UnitOff<N> u[(N - 1) * (N - 2) / 2];
-    __host__ __device__ static constexpr int index(int L, int la) { return (L - 1) * (L - 2) / 2 + la - 1; }
+template <int N, int W>
+constexpr int flat_count_ops()
+{
+    constexpr int M = N - 1;
+    constexpr LevelProgram<N, W> p = LevelProgramOf<N, W>::value;
+    int n = 0;
+    for (int L = 2; L <= M; ++L)
+        for (int w = 0; w < W; ++w) {
+            int here = 0;
+            for (int t = p.beg[L][w]; t < p.beg[L][w + 1]; ++t) {
+                const uint32_t a = p.task[t].a;
+                const int lo = a >> 4 & 15u, hi = a >> 8 & 15u;
+                here += (a & (LT_FIN | LT_PART)) && hi > lo ? hi - lo : 1;
+            }
+            n += here ? here : 1;                               // every warp takes the level-end barrier
+        }
+    return n;
+}
+
+template <int N, int W>
+struct FlatProgram {
+    static constexpr int NOPS = flat_count_ops<N, W>();
+    static constexpr int NQUAD = N * (N - 1) * (N - 2) * (N - 3) / 24;
+    FlatOp op[NOPS];
+    uint32_t quad[NQUAD > 0 ? NQUAD : 1];     // row J(k+1..l) | row J(l+1..j) << 16 per 4-gluon split
+    uint16_t beg[W + 1];                      // ops of warp w: [beg[w], beg[w+1])
 };
 
 template <class F, int N, int D, int W, int S>
-constexpr UnitTable<N> make_unit_table()
+constexpr FlatProgram<N, W> make_flat_program()
 {
-    typedef TileCfg<F, N, D, W, S> C;
-    UnitTable<N> t{};
-    constexpr int M = N - 1;
-    constexpr int EB = (int)sizeof(typename F::E), TP = C::TP;
-    for (int L = 2; L <= M; ++L)
-        for (int la = 1; la <= L - 1; ++la) {
-            UnitOff<N>& o = t.u[UnitTable<N>::index(L, la)];
-            const int ra = lv_rowbase<N>(la), rb = lv_rowbase<N>(L - la) + la;
-            o.a = (uint16_t)(ra * D * EB);
-            o.b = (uint16_t)(rb * D * EB);
-            o.ps = (uint16_t)((C::PS0 + la) * D * EB);
-            o.u = (uint32_t)((C::SC_U + ra) * TP * EB);
-            o.v = (uint32_t)((C::SC_V + rb) * TP * EB);
-            o.own = (uint16_t)(lv_rowbase<N>(L) * D * EB);
-            o.w = (uint32_t)((C::SC_W + lv_rowbase<N>(L) - N) * TP * EB);
-            for (int lb = 1; lb <= L - la - 1; ++lb) {
-                o.bm[lb - 1] = (uint16_t)((lv_rowbase<N>(lb) + la) * D * EB);
-                o.c[lb - 1] = (uint16_t)((lv_rowbase<N>(L - la - lb) + la + lb) * D * EB);
+    typedef TileCfg<F, N, D, W, S, false> C;    // only what does not depend on KW is used below
+    constexpr int M = N - 1, EB = (int)sizeof(typename F::E), TP = C::TP, RB = D * EB;
+    static_assert((long)C::VEC_ROWS * RB < 65536, "row offsets are 16-bit");
+    constexpr LevelProgram<N, W> p = LevelProgramOf<N, W>::value;
+    FlatProgram<N, W> f{};
+    int no = 0, nq = 0;
+    for (int w = 0; w < W; ++w) {
+        f.beg[w] = (uint16_t)no;
+        for (int L = 2; L <= M; ++L) {
+            const int first = no;
+            for (int t = p.beg[L][w]; t < p.beg[L][w + 1]; ++t) {
+                const uint32_t a = p.task[t].a, mask = p.task[t].mask;
+                const int ci = a & 15u, lo = a >> 4 & 15u, hi = a >> 8 & 15u, slot = a >> 12 & 63u;
+                const uint32_t bar = (a & LT_BAR) ? OP_BAR : 0u;
+                if (!(a & (LT_FIN | LT_PART))) {                // bare barrier
+                    f.op[no].qcf = bar << 24;
+                    ++no;
+                    continue;
+                }
+                const int own = lv_rowbase<N>(L) + ci;
+                const uint32_t endf = ((a & LT_PART) ? OP_PART : OP_FIN) | (L == M ? OP_TOP : 0u);
+                const uint32_t wfield = (uint32_t)(ci * M + ci + L - 1) | (uint32_t)own << 16;
+                const uint32_t lh = (uint32_t)((C::PS0 + ci) * RB) | (uint32_t)((C::PS0 + ci + L) * RB) << 16;
+                const uint32_t aux = (a & LT_PART) ? (uint32_t)(slot * (D + 1) * TP * EB) : mask;
+                if (hi == lo) {                                 // gather op
+                    FlatOp& o = f.op[no++];
+                    o.pso = (uint32_t)(own * RB) << 16;
+                    o.w = wfield;
+                    o.lh = lh;
+                    o.qcf = (bar | OP_START | OP_GATHER | endf) << 24;
+                    o.aux = aux;
+                    continue;
+                }
+                for (int la = lo + 1; la <= hi; ++la) {
+                    FlatOp& o = f.op[no++];
+                    const int ra = lv_rowbase<N>(la) + ci, rb = lv_rowbase<N>(L - la) + ci + la, c4 = L - la - 1;
+                    o.ab = (uint32_t)(ra * RB) | (uint32_t)(rb * RB) << 16;
+                    o.pso = (uint32_t)((C::PS0 + ci + la) * RB) | (uint32_t)(own * RB) << 16;
+                    o.u = (uint32_t)((C::SC_U + ra) * TP * EB);
+                    o.v = (uint32_t)(C::v_index(rb) * TP * EB);
+                    o.w = wfield;
+                    o.lh = lh;
+                    o.aux = aux;
+                    const uint32_t fl = OP_UNIT | (la == lo + 1 ? bar | OP_START : 0u) | (la == hi ? endf : 0u);
+                    o.qcf = (uint32_t)nq | (uint32_t)c4 << 16 | fl << 24;
+                    for (int lb = 1; lb <= c4; ++lb)
+                        f.quad[nq++] = (uint32_t)((lv_rowbase<N>(lb) + ci + la) * RB) |
+                                       (uint32_t)((lv_rowbase<N>(L - la - lb) + ci + la + lb) * RB) << 16;
+                }
             }
+            if (no == first) f.op[no++].qcf = 0;               // nothing to do at this level but the barrier
+            if (L < M) f.op[no - 1].qcf |= OP_LEND << 24;
         }
-    return t;
+    }
+    f.beg[W] = (uint16_t)no;
+    return f;
 }
 
 template <class F, int N, int D, int W, int S>
-__constant__ UnitTable<N> c_unit_table = make_unit_table<F, N, D, W, S>();
+__constant__ FlatProgram<N, W> c_flat_program = make_flat_program<F, N, D, W, S>();
 
-// one unit with C4 4-gluon splits; entry and exit: every acc[] has room for kCapR more products
-template <class F, int MET, int N, int D, int S, int C4>
-__device__ __forceinline__ void unit_body(const F& f, int mu0, const typename F::E* __restrict__ ri,
-                                          const typename F::E* __restrict__ si, const UnitOff<N>& o,
-                                          const typename F::E (&x2)[D / S], typename F::A (&acc)[D / S],
-                                          typename F::E& hsum)
+// the 4-gluon split (i..k | k+1..l | l+1..j): acc += 2 (A.C) J(k+1..l); na = -g A
+template <class F, int D, int S>
+__device__ __forceinline__ void unit_quad(const F& f, const char* __restrict__ rb_, uint32_t bc,
+                                          const typename F::E (&na)[D / S], typename F::A (&acc)[D / S])
 {
     typedef typename F::E E;
     constexpr int DL = D / S, TP = 32 / S;
-    const char* rb_ = reinterpret_cast<const char*>(ri);
-    const char* sb_ = reinterpret_cast<const char*>(si);
+    E bm[DL], c[DL];
+    ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (bc & 0xffffu)), bm);
+    ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (bc >> 16)), c);
+    const E cc = f.neg(f.dbl(lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, na, c)))));
+#pragma unroll
+    for (int mu = 0; mu < DL; ++mu) acc[mu] = f.mad(cc, bm[mu], acc[mu]);
+}
+
+// one unit: the 3-gluon split (A | B) and its c4 4-gluon splits; entry and exit: every acc[] has room for
+// kCapR more products.  The 4-gluon splits are a run-time loop over pairs (the relief pattern of a pair is
+// static), so there is ONE body for every c4 and the kernel stays inside the instruction cache for any n.
+template <class F, int MET, int N, int D, int S>
+__device__ __forceinline__ void unit_body(const F& f, int mu0, const typename F::E* __restrict__ rec,
+                                          const typename F::E* __restrict__ sc, const FlatOp& o,
+                                          const uint32_t* __restrict__ quad, const typename F::E (&x2)[D / S],
+                                          typename F::A (&acc)[D / S], typename F::E& hsum)
+{
+    typedef typename F::E E;
+    constexpr int DL = D / S, TP = 32 / S;
+    static_assert(F::kCapR >= 2, "the relief pattern below assumes room for two products after relief()");
+    const char* rb_ = reinterpret_cast<const char*>(rec);
+    const char* sb_ = reinterpret_cast<const char*>(sc);
     E a[DL], b[DL], s[DL], na[DL];
-    ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + o.a), a);
-    ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + o.b), b);
-    ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + o.ps), s);      // PS2_k, k = i+la-1
+    ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (o.ab & 0xffffu)), a);
+    ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (o.ab >> 16)), b);
+    ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (o.pso & 0xffffu)), s);      // PS2_k, k = i+la-1
     const E ua = *reinterpret_cast<const E*>(sb_ + o.u), vb = *reinterpret_cast<const E*>(sb_ + o.v);
     lower_neg<F, MET, DL>(f, mu0, a, na);
     const E h = f.neg(lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, na, b))));   // A.B
@@ -91,75 +175,48 @@ __device__ __forceinline__ void unit_body(const F& f, int mu0, const typename F:
     const E cb = f.sub(xa, ua);
     const E ca = f.sub(vb, xb);
     hsum = f.add(hsum, h);
-    int room = F::kCapR;
-    auto need = [&](int k) {
-        if (room < k) {
+    auto relieve = [&]() {
 #pragma unroll
-            for (int mu = 0; mu < DL; ++mu) acc[mu] = f.relief(acc[mu]);
-            room = F::kCapR;
-        }
-        room -= k;
+        for (int mu = 0; mu < DL; ++mu) acc[mu] = f.relief(acc[mu]);
     };
-    need(2);
 #pragma unroll
     for (int mu = 0; mu < DL; ++mu) {
         acc[mu] = f.mad(h, s[mu], acc[mu]);
         acc[mu] = f.mad(cb, b[mu], acc[mu]);
     }
-    need(1);
+    if (F::kExact) relieve();
 #pragma unroll
-    for (int mu = 0; mu < DL; ++mu) acc[mu] = f.mad(ca, a[mu], acc[mu]);
-#pragma unroll
-    for (int q = 0; q < C4; ++q) {
-        // (i..k | k+1..l | l+1..j), l = k+q+1: 2 (A.C) J(k+1..l)
-        E bm[DL], c[DL];
-        ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + o.bm[q]), bm);
-        ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + o.c[q]), c);
-        const E cc = f.neg(f.dbl(lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, na, c)))));
-        need(1);
-#pragma unroll
-        for (int mu = 0; mu < DL; ++mu) acc[mu] = f.mad(cc, bm[mu], acc[mu]);
+    for (int mu = 0; mu < DL; ++mu) acc[mu] = f.mad(ca, a[mu], acc[mu]);      // room for one more product
+    const int c4 = o.qcf >> 16 & 0xffu;
+    const uint32_t* qd = quad + (o.qcf & 0xffffu);
+    int q = 0;
+#pragma unroll 1
+    for (; q + 2 <= c4; q += 2) {
+        unit_quad<F, D, S>(f, rb_, qd[q], na, acc);
+        if (F::kExact) relieve();
+        unit_quad<F, D, S>(f, rb_, qd[q + 1], na, acc);                      // room for one more product again
     }
-    if (room < F::kCapR) {
-#pragma unroll
-        for (int mu = 0; mu < DL; ++mu) acc[mu] = f.relief(acc[mu]);
+    if (q < c4) {
+        unit_quad<F, D, S>(f, rb_, qd[q], na, acc);
     }
+    if (F::kExact) relieve();
 }
 
-// dispatch on the (warp-uniform) number of 4-gluon splits
-template <class F, int MET, int N, int D, int S, int C4>
-struct UnitDispatch {
-    __device__ __forceinline__ static void run(const F& f, int mu0, int c4, const typename F::E* __restrict__ ri,
-                                               const typename F::E* __restrict__ si, const UnitOff<N>& o,
-                                               const typename F::E (&x2)[D / S], typename F::A (&acc)[D / S],
-                                               typename F::E& hsum)
-    {
-        if (c4 == C4) unit_body<F, MET, N, D, S, C4>(f, mu0, ri, si, o, x2, acc, hsum);
-        else UnitDispatch<F, MET, N, D, S, C4 - 1>::run(f, mu0, c4, ri, si, o, x2, acc, hsum);
-    }
-};
-template <class F, int MET, int N, int D, int S>
-struct UnitDispatch<F, MET, N, D, S, -1> {
-    __device__ __forceinline__ static void run(const F&, int, int, const typename F::E*, const typename F::E*,
-                                               const UnitOff<N>&, const typename F::E (&)[D / S],
-                                               typename F::A (&)[D / S], typename F::E&)
-    {
-    }
-};
-
-// Finish the current (ci, L) whose bracket sum is in acc (room for kCapR more products): boundary
-// term of the (P-Q) sum, propagator, store, U and V; for the top current the amplitude instead
-// (no propagator).  The ONE copy of this block (every kernel variant of round 1 had its own).
-template <class F, int MET, int N, int D, int W, int S>
-__device__ __forceinline__ void unit_finish(const F& f, const TileLane<F, N, D, W, S>& t, typename F::E* ri,
-                                            typename F::E* si, const typename F::E (&l)[D / S],
-                                            const typename F::E (&h)[D / S], const typename F::E (&x2)[D / S],
-                                            typename F::A (&acc)[D / S], typename F::E hsum, int ci, int L, int own,
-                                            int widx, typename F::E* out, typename F::E* currents)
+// Finish the current whose bracket sum is in acc (room for kCapR more products): boundary term of the (P-Q)
+// sum, propagator, store, U and V; for the top current the amplitude instead (no propagator).
+template <class F, int MET, int N, int D, int W, int S, bool KW>
+__device__ __forceinline__ void unit_finish(const F& f, const TileLane<F, N, D, W, S, KW>& t, typename F::E* rec,
+                                            typename F::E* sc, const FlatOp& o, bool top,
+                                            const typename F::E (&x2)[D / S], typename F::A (&acc)[D / S],
+                                            typename F::E hsum, typename F::E* out, typename F::E* currents)
 {
-    typedef TileCfg<F, N, D, W, S> C;
+    typedef TileCfg<F, N, D, W, S, KW> C;
     typedef typename F::E E;
     constexpr int M = N - 1, DL = C::DL, TP = C::TP;
+    char* rb_ = reinterpret_cast<char*>(rec);
+    E l[DL], h[DL];
+    ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (o.lh & 0xffffu)), l);     // PS2_{i-1}
+    ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (o.lh >> 16)), h);         // PS2_j
     const E nhh = f.neg(f.mul(hsum, f.half()));                 // -(sum_k h_k)/2
     if constexpr (F::kExact) {
         // one product per component: the two ALU instructions of the add are cheaper than a
@@ -174,97 +231,93 @@ __device__ __forceinline__ void unit_finish(const F& f, const TileLane<F, N, D, 
         }
     }
     E v[DL];
-    if (L < M) {
-        const E w = *reinterpret_cast<const E*>(reinterpret_cast<const char*>(si) + widx);
+    if (!top) {
+        const uint32_t own = o.pso >> 16, urow = o.w >> 16;
+        const E w = sc[(C::SC_W + urow - N) * TP];              // 1/P^2
 #pragma unroll
         for (int mu = 0; mu < DL; ++mu) v[mu] = f.mul(f.reduce(acc[mu]), w);
-        st_vec<F, DL>(reinterpret_cast<E*>(reinterpret_cast<char*>(ri) + own), v);
+        st_vec<F, DL>(reinterpret_cast<E*>(rb_ + own), v);
         const E c2 = lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, x2, v)));    // 2 P_{i,j} . J(i..j)
-        const int urow = own / (D * (int)sizeof(E));
-        si[(C::SC_U + urow) * TP] = f.add(c2, hsum);
-        si[(C::SC_V + urow) * TP] = f.sub(c2, hsum);
+        sc[(C::SC_U + urow) * TP] = f.add(c2, hsum);
+        sc[(C::SC_V + urow - N) * TP] = f.sub(c2, hsum);
     } else {
 #pragma unroll
         for (int mu = 0; mu < DL; ++mu) v[mu] = f.reduce(acc[mu]);
         E e[DL], ne[DL];
-        ld_vec<F, DL>(t.rec() + (N - 1) * D, e);
+        ld_vec<F, DL>(rec + (N - 1) * D, e);
         lower_neg<F, MET, DL>(f, t.mu0, e, ne);
         const E nout = lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, ne, v)));  // -(eps_n . N)
         if (t.live && t.half == 0) *out = f.to_output(f.neg(nout));
     }
     if (currents && t.live) {
-        E* dst = currents + (t.pt * M * M + (long long)ci * M + (ci + L - 1)) * D + t.mu0;
+        E* dst = currents + (t.pt * M * M + (long long)(o.w & 0xffffu)) * D + t.mu0;
 #pragma unroll
         for (int mu = 0; mu < DL; ++mu) dst[mu] = f.to_output(v[mu]);
     }
 }
 
 // a4-a6 for one state configuration of one tile: the level sweep L = 2..m (Eq.(6)), amplitude, store.
-template <class F, int MET, int N, int D, int W, int S>
-__device__ __forceinline__ void unit_sweep_body(const F& f, const TileLane<F, N, D, W, S>& t, const int warp,
+template <class F, int MET, int N, int D, int W, int S, bool KW>
+__device__ __forceinline__ void unit_sweep_body(const F& f, const TileLane<F, N, D, W, S, KW>& t, const int warp,
                                                 typename F::E* out, typename F::E* currents)
 {
-    typedef TileCfg<F, N, D, W, S> C;
+    typedef TileCfg<F, N, D, W, S, KW> C;
     typedef typename F::E E;
     typedef typename F::A A;
-    constexpr int M = N - 1, DL = C::DL, TP = C::TP;
-    const LevelProgram<N, W>& tb = c_level_program<F, N, D, W>;
-    const UnitTable<N>& ut = c_unit_table<F, N, D, W, S>;
+    constexpr int DL = C::DL, TP = C::TP;
+    const FlatProgram<N, W>& fp = c_flat_program<F, N, D, W, S>;
     E* rec = t.rec();
     E* sc = t.sc();
-    // ---- a4-a6: level sweep L = 2..m (Eq.(6)), amplitude, store --------------------
+    char* rb_ = reinterpret_cast<char*>(rec);
+    char* sb_ = reinterpret_cast<char*>(sc);
+    E x2[DL];
+    A acc[DL];
+    E hsum = f.ezero();
+#pragma unroll
+    for (int mu = 0; mu < DL; ++mu) { x2[mu] = f.ezero(); acc[mu] = f.zero(); }
+    const int k0 = fp.beg[warp], k1 = fp.beg[warp + 1];
 #pragma unroll 1
-    for (int L = 2; L <= M; ++L) {
-        const int lbase = UnitTable<N>::index(L, 1);
-        const int own = ut.u[lbase].own, widx = ut.u[lbase].w;
-        const int t0 = tb.beg[L][warp], t1 = tb.beg[L][warp + 1];
-#pragma unroll 1
-        for (int k = t0; k < t1; ++k) {
-            const uint32_t ta = tb.task[k].a;
-            if (ta & LT_BAR) __syncthreads();
-            if (!(ta & (LT_FIN | LT_PART))) continue;
-            const int ci = ta & 15u, lo = ta >> 4 & 15u, hi = ta >> 8 & 15u;
-            E* ri = rec + ci * D;
-            E* si = sc + ci * TP;
-            E l[DL], h[DL], x2[DL];
-            ld_vec<F, DL>(ri + C::PS0 * D, l);                     // PS2_{i-1}
-            ld_vec<F, DL>(ri + (C::PS0 + L) * D, h);               // PS2_j
-            lower_diff<F, MET, DL>(f, t.mu0, h, l, x2);            // 2 * covariant P_{i,j}
-            A acc[DL];
+    for (int k = k0; k < k1; ++k) {
+        const FlatOp& o = fp.op[k];
+        const uint32_t fl = o.qcf >> 24;
+        if (fl & OP_BAR) __syncthreads();
+        if (fl & OP_START) {
+            E l[DL], h[DL];
+            ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (o.lh & 0xffffu)), l);     // PS2_{i-1}
+            ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (o.lh >> 16)), h);         // PS2_j
+            lower_diff<F, MET, DL>(f, t.mu0, h, l, x2);                               // 2 * covariant P_{i,j}
 #pragma unroll
             for (int mu = 0; mu < DL; ++mu) acc[mu] = f.zero();
-            E hsum = f.ezero();
-#pragma unroll 1
-            for (int la = lo + 1; la <= hi; ++la)
-                UnitDispatch<F, MET, N, D, S, N - 3>::run(f, t.mu0, L - la - 1, ri, si, ut.u[lbase + la - 1], x2,
-                                                          acc, hsum);
-            uint32_t mask = tb.task[k].mask;
-            if (mask) {                                            // gather task (no units of its own)
-                E sum[DL];
-#pragma unroll
-                for (int mu = 0; mu < DL; ++mu) sum[mu] = f.ezero();
-                while (mask) {
-                    const int slot = __ffs(mask) - 1;
-                    mask &= mask - 1;
-                    const E* scr = sc + (C::SC_SCR + slot * (D + 1)) * TP;
-#pragma unroll
-                    for (int mu = 0; mu < DL; ++mu) sum[mu] = f.add(sum[mu], scr[(t.mu0 + mu) * TP]);
-                    hsum = f.add(hsum, scr[D * TP]);
-                }
-#pragma unroll
-                for (int mu = 0; mu < DL; ++mu) acc[mu] = f.widen(sum[mu]);
-            }
-            if (ta & LT_PART) {
-                E* scr = sc + (C::SC_SCR + (ta >> 12 & 63u) * (D + 1)) * TP;
-#pragma unroll
-                for (int mu = 0; mu < DL; ++mu) scr[(t.mu0 + mu) * TP] = f.reduce(acc[mu]);
-                scr[D * TP] = hsum;
-                continue;
-            }
-            unit_finish<F, MET, N, D, W, S>(f, t, ri, si, l, h, x2, acc, hsum, ci, L, own, widx, out,
-                                            currents);
+            hsum = f.ezero();
         }
-        if (L < M) __syncthreads();
+        if (fl & OP_UNIT) unit_body<F, MET, N, D, S>(f, t.mu0, rec, sc, o, fp.quad, x2, acc, hsum);
+        if (fl & OP_GATHER) {
+            uint32_t mask = o.aux;
+            E sum[DL];
+#pragma unroll
+            for (int mu = 0; mu < DL; ++mu) sum[mu] = f.ezero();
+            while (mask) {
+                const int slot = __ffs(mask) - 1;
+                mask &= mask - 1;
+                const E* scr = sc + (C::SC_SCR + slot * (D + 1)) * TP;
+#pragma unroll
+                for (int mu = 0; mu < DL; ++mu) sum[mu] = f.add(sum[mu], scr[(t.mu0 + mu) * TP]);
+                hsum = f.add(hsum, scr[D * TP]);
+            }
+#pragma unroll
+            for (int mu = 0; mu < DL; ++mu) acc[mu] = f.widen(sum[mu]);
+        }
+        if (fl & OP_PART) {
+            // (a byte offset from the table, not slot * (D + 1): a run-time multiply here makes ptxas give up the
+            // uniform datapath for the whole sweep, +4.5 % at cfg2)
+            E* scr = reinterpret_cast<E*>(sb_ + C::SC_SCR * TP * (int)sizeof(E) + o.aux);
+#pragma unroll
+            for (int mu = 0; mu < DL; ++mu) scr[(t.mu0 + mu) * TP] = f.reduce(acc[mu]);
+            scr[D * TP] = hsum;
+        }
+        if (fl & OP_FIN)
+            unit_finish<F, MET, N, D, W, S, KW>(f, t, rec, sc, o, (fl & OP_TOP) != 0, x2, acc, hsum, out, currents);
+        if (fl & OP_LEND) __syncthreads();
     }
 }
 
@@ -275,22 +328,20 @@ __device__ __forceinline__ void unit_sweep_body(const F& f, const TileLane<F, N,
 // as a __noinline__ function from the loops brings part of the uniform code back but costs more than it saves:
 // S = 4 at cfg2's shape 1.00 -> 1.15 ms.)
 template <class F, int MET, int N, int D, int W, int S, bool MULTI>
-__global__ void __launch_bounds__(32 * W, TileCfg<F, N, D, W, S>::MIN_BLOCKS) bg_unit_kernel(const BgParams<F> prm)
+__global__ void __launch_bounds__(32 * W, TileCfg<F, N, D, W, S, MULTI>::MIN_BLOCKS) bg_unit_kernel(const BgParams<F> prm)
 {
-    typedef TileCfg<F, N, D, W, S> C;
-    typedef TileSetup<F, N, D, W, S> Setup;
+    constexpr bool KW = MULTI;
+    typedef TileCfg<F, N, D, W, S, KW> C;
+    typedef TileSetup<F, N, D, W, S, KW> Setup;
     typedef typename F::E E;
     typedef typename F::A A;
     constexpr int M = N - 1, ND = N * D, DL = C::DL, TP = C::TP;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const F f(prm.fld, blockIdx.y);
-    TileLane<F, N, D, W, S> t;
+    TileLane<F, N, D, W, S, KW> t;
     t.vec = reinterpret_cast<E*>(smem_raw);                   // [TP][VSTRIDE]
     t.scal = t.vec + TP * C::VSTRIDE;                         // [NSCAL][TP]
     t.stat = reinterpret_cast<uint32_t*>(t.scal + TP * C::NSCAL);
-    const LevelProgram<N, W>& tb = c_level_program<F, N, D, W>;
-    const UnitTable<N>& ut = c_unit_table<F, N, D, W, S>;
-
     // the warp index, broadcast from lane 0 so that everything derived from it (task bounds,
     // task words, branch conditions) is compiled as warp-uniform
     const int lane = threadIdx.x & 31;
@@ -323,8 +374,8 @@ __global__ void __launch_bounds__(32 * W, TileCfg<F, N, D, W, S>::MIN_BLOCKS) bg
     const unsigned char* perm = MULTI && prm.orderings ? prm.orderings + o * N : nullptr;
     if (o > 0) __syncthreads();                                // the previous sweep is done with the record
     // ---- a0: stage the momenta k_1..k_m (k_n is never used) and the first state configuration ----
-    tile_stage<F, N, D, W, S, Setup::PARK, M>(f, t, gmom, ND, perm);
-    tile_stage<F, N, D, W, S, 0, N>(f, t, gpol, (long long)states * ND, perm);
+    tile_stage<F, N, D, W, S, KW, Setup::PARK, M>(f, t, gmom, ND, perm);
+    tile_stage<F, N, D, W, S, KW, 0, N>(f, t, gpol, (long long)states * ND, perm);
     __syncthreads();
     // ---- a1-a3: prefix sums, invariants, propagators (momenta only: once per tile and ordering) ----
     Setup::prefix(f, t);
@@ -335,13 +386,13 @@ __global__ void __launch_bounds__(32 * W, TileCfg<F, N, D, W, S>::MIN_BLOCKS) bg
     for (int s = 0; s < states; ++s) {
         if (s > 0) {
             __syncthreads();                                   // the previous sweep is done with eps_n
-            tile_stage<F, N, D, W, S, 0, N>(f, t, gpol + (long long)s * ND, (long long)states * ND, perm);
+            tile_stage<F, N, D, W, S, KW, 0, N>(f, t, gpol + (long long)s * ND, (long long)states * ND, perm);
             __syncthreads();
             Setup::template singles<MET>(f, t, prm.currents);
             __syncthreads();
         }
 
-        unit_sweep_body<F, MET, N, D, W, S>(f, t, warp, gout + s, prm.currents);
+        unit_sweep_body<F, MET, N, D, W, S, KW>(f, t, warp, gout + s, prm.currents);
     }
     }
 }
