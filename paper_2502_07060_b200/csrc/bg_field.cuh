@@ -70,6 +70,8 @@ struct Fp31 {
     __device__ __forceinline__ A mad(E a, E b, A c) const { return (uint64_t)a * b + c; }
     // accumulator holding the element a (counts as one product for the headroom rules)
     __device__ __forceinline__ A widen(E a) const { return (uint64_t)a; }
+    // accumulator + element (counts as one product)
+    __device__ __forceinline__ A addw(A x, E a) const { return x + (uint64_t)a; }
     // Headroom without touching the multiplier pipe (header comment): ONE ALU instruction.
     __device__ __forceinline__ A relief(A x) const
     {
@@ -177,6 +179,7 @@ struct FpMont {
     __device__ __forceinline__ A mad(E a, E b, A c) const { return (uint64_t)a * b + c; }
     // accumulators hold products of two Montgomery forms (scale R^2): an element enters as a * R
     __device__ __forceinline__ A widen(E a) const { return (uint64_t)a * one_; }
+    __device__ __forceinline__ A addw(A x, E a) const { return (uint64_t)a * one_ + x; }
     __device__ __forceinline__ A relief(A x) const
     {
         uint32_t lo, hi;
@@ -241,6 +244,7 @@ struct C128 {
         return make_double2(re, im);
     }
     __device__ __forceinline__ A widen(E a) const { return a; }
+    __device__ __forceinline__ A addw(A x, E a) const { return make_double2(x.x + a.x, x.y + a.y); }
     __device__ __forceinline__ A relief(A x) const { return x; }
     __device__ __forceinline__ E reduce(A x) const { return x; }
     __device__ __forceinline__ E neg(E a) const { return make_double2(-a.x, -a.y); }

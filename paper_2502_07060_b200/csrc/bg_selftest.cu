@@ -2,9 +2,11 @@
 //
 // The level sweep of Eq.(6) is driven by constexpr task lists (make_level_program in
 // bg_schedule.cuh).  bg_selftest_schedules() rebuilds the same lists on the host and checks, for every compiled
-// (n, warps) pair, that every splitting of every current is executed exactly once, that a
-// current is either finished by the warp that owns all of it or has its parts gathered exactly
-// once from distinct scratch slots, and that the barriers of a level are taken by every warp.
+// (n, warps) pair, that every splitting of every current is executed exactly once; that a current is either
+// finished by the warp that owns all of it, or by the owner of its first units as the LAST task of that warp,
+// with every other part the FIRST task of another warp, parked in a scratch slot of its own that the finisher
+// adds exactly once; and that finisher and parts agree on the named barrier and on the number of warps that
+// meet there (a mismatch would hang the block).
 // Pure host code: callable without a GPU (tests/test_abi.py).
 #include <stdint.h>
 
@@ -15,7 +17,6 @@ namespace {
 
 using namespace bg;
 
-// ---- bg_schedule.cuh task lists --------------------------------------------------------------------
 template <int N, int W>
 int check_level_program()
 {
@@ -25,36 +26,39 @@ int check_level_program()
     for (int L = 2; L <= M; ++L) {
         const int NU = L - 1, NC = M - L + 1;
         int covered[16][16] = {};          // [ci][unit] -> times executed
-        int fin[16] = {}, parts[16] = {};
-        uint32_t part_slots[16] = {}, gather_mask[16] = {};
-        uint32_t level_slots = 0;
-        int bars[W] = {};
-        bool any_gather = false;
+        int fin[16] = {}, parts[16] = {}, fin_bar[16] = {}, fin_nwarps[16] = {}, part_bar_ok[16] = {};
+        uint32_t part_slots[16] = {}, fin_mask[16] = {};
+        uint32_t level_slots = 0, level_bars = 0;
         if (p.beg[L][0] != prev_end) return -100 - L;                       // lists are contiguous
         for (int w = 0; w < W; ++w) {
             if (p.beg[L][w + 1] < p.beg[L][w]) return -200 - L;
-            bool seen_bar = false;
             for (int t = p.beg[L][w]; t < p.beg[L][w + 1]; ++t) {
-                const uint32_t a = p.task[t].a, mask = p.task[t].mask;
+                const LevelTask& k = p.task[t];
+                const uint32_t a = k.a;
                 const int ci = a & 15u, lo = a >> 4 & 15u, hi = a >> 8 & 15u, slot = a >> 12 & 63u;
-                if (a & LT_BAR) { ++bars[w]; seen_bar = true; }
-                if (!(a & (LT_FIN | LT_PART))) continue;
-                if (ci >= NC || lo > hi || hi > NU) return -300 - L;
+                const bool first = t == p.beg[L][w], last = t + 1 == p.beg[L][w + 1];
+                if (!(a & (LT_FIN | LT_PART)) || ((a & LT_FIN) && (a & LT_PART))) return -250 - L;
+                if (ci >= NC || lo >= hi || hi > NU) return -300 - L;
                 for (int u = lo; u < hi; ++u) ++covered[ci][u];
                 if (a & LT_PART) {
-                    if (seen_bar || mask || lo == hi) return -400 - L;    // parts come before the barrier
+                    if (lo == 0 || !first || k.mask) return -400 - L;     // later parts are first tasks
                     if (slot >= p.nslots || (level_slots >> slot & 1u)) return -500 - L;
                     level_slots |= 1u << slot;
                     part_slots[ci] |= 1u << slot;
                     ++parts[ci];
+                    if (fin[ci] != 1 || k.bar != fin_bar[ci] || k.nwarps != fin_nwarps[ci]) return -550 - L;
+                    ++part_bar_ok[ci];
                 } else {
                     ++fin[ci];
-                    if (mask) {                                             // gather task
-                        if (!seen_bar || lo != hi) return -600 - L;
-                        gather_mask[ci] = mask;
-                        any_gather = true;
-                    } else if (lo != 0 || hi != NU || seen_bar) {
-                        return -700 - L;                                    // inline finish owns the whole current
+                    if (lo != 0) return -600 - L;
+                    if (hi < NU) {                                          // finisher of a shared current
+                        if (!last || !k.mask || k.bar < 1 || k.bar > 15 || (level_bars >> k.bar & 1u)) return -650 - L;
+                        level_bars |= 1u << k.bar;
+                        fin_mask[ci] = k.mask;
+                        fin_bar[ci] = k.bar;
+                        fin_nwarps[ci] = k.nwarps;
+                    } else if (k.mask || k.bar || k.nwarps) {
+                        return -700 - L;
                     }
                 }
             }
@@ -63,10 +67,10 @@ int check_level_program()
             for (int u = 0; u < NU; ++u)
                 if (covered[ci][u] != 1) return -800 - L;
             if (fin[ci] != 1) return -900 - L;
-            if (parts[ci] == 1 || part_slots[ci] != gather_mask[ci]) return -1000 - L;
+            if (part_slots[ci] != fin_mask[ci]) return -1000 - L;
+            if (parts[ci] && fin_nwarps[ci] != parts[ci] + 1) return -1100 - L;
+            if (parts[ci] > W - 1) return -1200 - L;
         }
-        for (int w = 0; w < W; ++w)
-            if (bars[w] != (any_gather ? 1 : 0)) return -1100 - L;
         prev_end = p.beg[L][W];
     }
     return 0;

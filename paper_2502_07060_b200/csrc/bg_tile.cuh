@@ -50,7 +50,8 @@ struct TileCfg {
     static constexpr int NSLOTS = LevelProgramOf<N, W>::value.nslots;
     static constexpr int NSCAL = SC_SCR + NSLOTS * (D + 1);
     static constexpr int THREADS = 32 * W;
-    static constexpr size_t SMEM_BYTES = (size_t)TP * (VSTRIDE + NSCAL) * sizeof(E) + TP * sizeof(uint32_t);
+    // + the status word per point and one "parked" flag per (scratch slot, lane)
+    static constexpr size_t SMEM_BYTES = (size_t)TP * (VSTRIDE + NSCAL) * sizeof(E) + (TP + 32 * NSLOTS) * sizeof(uint32_t);
     // resident blocks per SM that shared memory allows (228 KB per SM, 1 KB reserved per block): the register
     // budget of the kernel is set so that registers do not lower it (__launch_bounds__ in bg_unit.cuh)
     static constexpr int SMEM_BLOCKS = (int)(233472 / (SMEM_BYTES + 1024)) < 1 ? 1 : (int)(233472 / (SMEM_BYTES + 1024));
@@ -83,7 +84,7 @@ struct TileLane {
     typedef typename F::E E;
     E* vec;               // [TP][VSTRIDE]
     E* scal;              // [NSCAL][TP]
-    uint32_t* stat;       // [TP]
+    uint32_t* stat;       // [TP], then the parked flags [NSLOTS][32]
     int warp, point, half, mu0, valid;
     long long tile0, pt;  // first point of the tile, this lane's point (index within the prime's batch)
     long long q;          // prime index (blockIdx.y)

@@ -23,12 +23,11 @@ namespace bg {
 // byte offset from the lane's record / scalar base, so the sweep is a single run-time loop whose body needs
 // two 16-byte constant loads and a few warp-uniform flag tests (round 2 decoded a task word, a unit-table
 // entry and a level header per iteration: 4.2 k of the 20.3 k instructions per cfg2 tile).
-constexpr uint32_t OP_BAR = 1u;       // block barrier before the op (first gather op of the level)
 constexpr uint32_t OP_START = 2u;     // first op of a task: form 2 P_{i,j}, clear the bracket sums
 constexpr uint32_t OP_UNIT = 4u;      // a 3-gluon split with its c4 4-gluon splits
-constexpr uint32_t OP_PART = 8u;      // last op of a task that owns part of a current: park the partial sums
+constexpr uint32_t OP_PART = 8u;      // last op of a later part of a shared current: park the partial sums, raise the flag
 constexpr uint32_t OP_FIN = 16u;      // last op of a task: finish the current
-constexpr uint32_t OP_GATHER = 32u;   // sum the parked partial sums (aux = mask of scratch slots)
+constexpr uint32_t OP_GATHER = 32u;   // finisher of a shared current: check the flags, add the parked sums (aux = slots)
 constexpr uint32_t OP_LEND = 64u;     // block barrier after the op (end of the level)
 constexpr uint32_t OP_TOP = 128u;     // the current is J(1..m): amplitude instead of propagator and store
 
@@ -36,7 +35,8 @@ struct FlatOp {
     uint32_t ab;       // row A | row B << 16      (byte offsets in the lane's vector record)
     uint32_t pso;      // row PS2_k | own row << 16
     uint32_t u, v;     // U_A, V_B                 (byte offsets from the lane's scalar base)
-    uint32_t w;        // ci * m + j - 1 (position of the current in the caller's `currents` array) | own row << 16
+    uint32_t w;        // ci * m + j - 1 (position in the caller's `currents` array) | own row << 8 | level << 16
+                       // | OP_PART: first parked flag of the slot (word index) << 20
     uint32_t lh;       // rows PS2_{i-1} | PS2_j << 16
     uint32_t qcf;      // first entry of the op's 4-gluon splits in quad[] | c4 << 16 | flags << 24
     uint32_t aux;      // OP_PART: scratch slot (byte offset from the first slot) ; OP_GATHER: mask of slots
@@ -53,8 +53,7 @@ constexpr int flat_count_ops()
             int here = 0;
             for (int t = p.beg[L][w]; t < p.beg[L][w + 1]; ++t) {
                 const uint32_t a = p.task[t].a;
-                const int lo = a >> 4 & 15u, hi = a >> 8 & 15u;
-                here += (a & (LT_FIN | LT_PART)) && hi > lo ? hi - lo : 1;
+                here += (int)(a >> 8 & 15u) - (int)(a >> 4 & 15u);          // one op per unit
             }
             n += here ? here : 1;                               // every warp takes the level-end barrier
         }
@@ -86,26 +85,14 @@ constexpr FlatProgram<N, W> make_flat_program()
             for (int t = p.beg[L][w]; t < p.beg[L][w + 1]; ++t) {
                 const uint32_t a = p.task[t].a, mask = p.task[t].mask;
                 const int ci = a & 15u, lo = a >> 4 & 15u, hi = a >> 8 & 15u, slot = a >> 12 & 63u;
-                const uint32_t bar = (a & LT_BAR) ? OP_BAR : 0u;
-                if (!(a & (LT_FIN | LT_PART))) {                // bare barrier
-                    f.op[no].qcf = bar << 24;
-                    ++no;
-                    continue;
-                }
                 const int own = lv_rowbase<N>(L) + ci;
-                const uint32_t endf = ((a & LT_PART) ? OP_PART : OP_FIN) | (L == M ? OP_TOP : 0u);
-                const uint32_t wfield = (uint32_t)(ci * M + ci + L - 1) | (uint32_t)own << 16;
+                const uint32_t endf = ((a & LT_PART) ? OP_PART : mask ? OP_GATHER | OP_FIN : OP_FIN) |
+                                      (L == M ? OP_TOP : 0u);
+                static_assert(M * M <= 256 && N + M * (M - 1) / 2 <= 256, "8-bit fields of FlatOp::w");
+                const uint32_t wfield = (uint32_t)(ci * M + ci + L - 1) | (uint32_t)own << 8 |
+                                        (uint32_t)L << 16 | ((a & LT_PART) ? (uint32_t)(32 * slot) << 20 : 0u);
                 const uint32_t lh = (uint32_t)((C::PS0 + ci) * RB) | (uint32_t)((C::PS0 + ci + L) * RB) << 16;
                 const uint32_t aux = (a & LT_PART) ? (uint32_t)(slot * (D + 1) * TP * EB) : mask;
-                if (hi == lo) {                                 // gather op
-                    FlatOp& o = f.op[no++];
-                    o.pso = (uint32_t)(own * RB) << 16;
-                    o.w = wfield;
-                    o.lh = lh;
-                    o.qcf = (bar | OP_START | OP_GATHER | endf) << 24;
-                    o.aux = aux;
-                    continue;
-                }
                 for (int la = lo + 1; la <= hi; ++la) {
                     FlatOp& o = f.op[no++];
                     const int ra = lv_rowbase<N>(la) + ci, rb = lv_rowbase<N>(L - la) + ci + la, c4 = L - la - 1;
@@ -116,7 +103,7 @@ constexpr FlatProgram<N, W> make_flat_program()
                     o.w = wfield;
                     o.lh = lh;
                     o.aux = aux;
-                    const uint32_t fl = OP_UNIT | (la == lo + 1 ? bar | OP_START : 0u) | (la == hi ? endf : 0u);
+                    const uint32_t fl = OP_UNIT | (la == lo + 1 ? OP_START : 0u) | (la == hi ? endf : 0u);
                     o.qcf = (uint32_t)nq | (uint32_t)c4 << 16 | fl << 24;
                     for (int lb = 1; lb <= c4; ++lb)
                         f.quad[nq++] = (uint32_t)((lv_rowbase<N>(lb) + ci + la) * RB) |
@@ -232,7 +219,7 @@ __device__ __forceinline__ void unit_finish(const F& f, const TileLane<F, N, D, 
     }
     E v[DL];
     if (!top) {
-        const uint32_t own = o.pso >> 16, urow = o.w >> 16;
+        const uint32_t own = o.pso >> 16, urow = o.w >> 8 & 0xffu;
         const E w = sc[(C::SC_W + urow - N) * TP];              // 1/P^2
 #pragma unroll
         for (int mu = 0; mu < DL; ++mu) v[mu] = f.mul(f.reduce(acc[mu]), w);
@@ -250,7 +237,7 @@ __device__ __forceinline__ void unit_finish(const F& f, const TileLane<F, N, D, 
         if (t.live && t.half == 0) *out = f.to_output(f.neg(nout));
     }
     if (currents && t.live) {
-        E* dst = currents + (t.pt * M * M + (long long)(o.w & 0xffffu)) * D + t.mu0;
+        E* dst = currents + (t.pt * M * M + (long long)(o.w & 0xffu)) * D + t.mu0;
 #pragma unroll
         for (int mu = 0; mu < DL; ++mu) dst[mu] = f.to_output(v[mu]);
     }
@@ -259,7 +246,7 @@ __device__ __forceinline__ void unit_finish(const F& f, const TileLane<F, N, D, 
 // a4-a6 for one state configuration of one tile: the level sweep L = 2..m (Eq.(6)), amplitude, store.
 template <class F, int MET, int N, int D, int W, int S, bool KW>
 __device__ __forceinline__ void unit_sweep_body(const F& f, const TileLane<F, N, D, W, S, KW>& t, const int warp,
-                                                typename F::E* out, typename F::E* currents)
+                                                const uint32_t epoch0, typename F::E* out, typename F::E* currents)
 {
     typedef TileCfg<F, N, D, W, S, KW> C;
     typedef typename F::E E;
@@ -270,6 +257,7 @@ __device__ __forceinline__ void unit_sweep_body(const F& f, const TileLane<F, N,
     E* sc = t.sc();
     char* rb_ = reinterpret_cast<char*>(rec);
     char* sb_ = reinterpret_cast<char*>(sc);
+    uint32_t* flags = t.stat + TP + (threadIdx.x & 31);         // this lane's parked flags, [slot * 32]
     E x2[DL];
     A acc[DL];
     E hsum = f.ezero();
@@ -280,7 +268,6 @@ __device__ __forceinline__ void unit_sweep_body(const F& f, const TileLane<F, N,
     for (int k = k0; k < k1; ++k) {
         const FlatOp& o = fp.op[k];
         const uint32_t fl = o.qcf >> 24;
-        if (fl & OP_BAR) __syncthreads();
         if (fl & OP_START) {
             E l[DL], h[DL];
             ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (o.lh & 0xffffu)), l);     // PS2_{i-1}
@@ -291,7 +278,28 @@ __device__ __forceinline__ void unit_sweep_body(const F& f, const TileLane<F, N,
             hsum = f.ezero();
         }
         if (fl & OP_UNIT) unit_body<F, MET, N, D, S>(f, t.mu0, rec, sc, o, fp.quad, x2, acc, hsum);
+        if (fl & OP_PART) {
+            // a later part of a current shared between warps: park the partial sums, tell the finisher.
+            // (a byte offset from the table, not slot * (D + 1): a run-time multiply here makes ptxas give up the
+            // uniform datapath for the whole sweep, +4.5 % at cfg2)
+            E* scr = reinterpret_cast<E*>(sb_ + C::SC_SCR * TP * (int)sizeof(E) + o.aux);
+#pragma unroll
+            for (int mu = 0; mu < DL; ++mu) scr[(t.mu0 + mu) * TP] = f.reduce(acc[mu]);
+            scr[D * TP] = hsum;
+            // the lane that reads a parked value is this lane of the finishing warp: a per-lane flag, raised after
+            // the values (fence), tells it that they are there; `epoch` is unique per sweep and level
+            __threadfence_block();
+            *reinterpret_cast<volatile uint32_t*>(flags + (o.w >> 20)) = epoch0 + (o.w >> 16 & 15u);
+        }
         if (fl & OP_GATHER) {
+            // the finisher (owner of the first units, this is its last task of the level): the other parts were
+            // first tasks of their warps and are parked by now
+            const uint32_t epoch = epoch0 + (o.w >> 16 & 15u);
+            for (uint32_t m2 = o.aux; m2; m2 &= m2 - 1) {
+                const volatile uint32_t* fl_ = flags + 32 * (__ffs(m2) - 1);
+                while (!__all_sync(0xffffffffu, *fl_ == epoch)) {}    // warp-uniform exit
+            }
+            __threadfence_block();
             uint32_t mask = o.aux;
             E sum[DL];
 #pragma unroll
@@ -305,15 +313,7 @@ __device__ __forceinline__ void unit_sweep_body(const F& f, const TileLane<F, N,
                 hsum = f.add(hsum, scr[D * TP]);
             }
 #pragma unroll
-            for (int mu = 0; mu < DL; ++mu) acc[mu] = f.widen(sum[mu]);
-        }
-        if (fl & OP_PART) {
-            // (a byte offset from the table, not slot * (D + 1): a run-time multiply here makes ptxas give up the
-            // uniform datapath for the whole sweep, +4.5 % at cfg2)
-            E* scr = reinterpret_cast<E*>(sb_ + C::SC_SCR * TP * (int)sizeof(E) + o.aux);
-#pragma unroll
-            for (int mu = 0; mu < DL; ++mu) scr[(t.mu0 + mu) * TP] = f.reduce(acc[mu]);
-            scr[D * TP] = hsum;
+            for (int mu = 0; mu < DL; ++mu) acc[mu] = f.addw(acc[mu], sum[mu]);   // one of the kCapR products of room
         }
         if (fl & OP_FIN)
             unit_finish<F, MET, N, D, W, S, KW>(f, t, rec, sc, o, (fl & OP_TOP) != 0, x2, acc, hsum, out, currents);
@@ -365,6 +365,8 @@ __global__ void __launch_bounds__(32 * W, TileCfg<F, N, D, W, S, MULTI>::MIN_BLO
     // (a warp-uniform condition first: after a thread-divergent branch in front of the barriers ptxas no longer
     // treats the sweep as convergent and gives up the uniform datapath for its control flow and table loads)
     if (warp == 0 && lane < TP) t.stat[lane] = 0;
+#pragma unroll 1
+    for (int sl = warp; sl < C::NSLOTS; sl += W) t.stat[TP + 32 * sl + lane] = 0;    // parked flags (epochs start at 1)
     E* rec = t.rec();
     E* sc = t.sc();
 #pragma unroll 1
@@ -392,7 +394,7 @@ __global__ void __launch_bounds__(32 * W, TileCfg<F, N, D, W, S, MULTI>::MIN_BLO
             __syncthreads();
         }
 
-        unit_sweep_body<F, MET, N, D, W, S, KW>(f, t, warp, gout + s, prm.currents);
+        unit_sweep_body<F, MET, N, D, W, S, KW>(f, t, warp, (uint32_t)(o * states + s) * 16u, gout + s, prm.currents);
     }
     }
 }
