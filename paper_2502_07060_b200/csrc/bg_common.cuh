@@ -13,6 +13,8 @@
 //
 // Per 3-split 3 dot products + 3 axpys, per 4-split 1 dot + 1 axpy.  Exact over F_p, hence
 // bit-identical to the literal evaluation; over complex128 a reordering within DESIGN.md R9/R10.
+// The tiled kernel accumulates MINUS the bracket (with -g A as the left factor of the Minkowski products and
+// -2 X, every coefficient but one comes out of its reduction with the right sign; the table holds -1/P^2).
 #pragma once
 #include "bg_field.cuh"
 
@@ -106,6 +108,21 @@ __device__ __forceinline__ typename F::A dot_plain(const F& f, const typename F:
 #pragma unroll
     for (int mu = 0; mu < D; ++mu) {
         if (mu >= F::kCap0 && ((mu - F::kCap0) % F::kCapR) == 0) s = f.relief(s);
+        s = f.mad(x[mu], y[mu], s);
+    }
+    return s;
+}
+
+// init + sum_mu x_mu y_mu (init an element: one more product for the headroom rules unless F::kWidenFree)
+template <class F, int D>
+__device__ __forceinline__ typename F::A dot_plain_from(const F& f, typename F::E init, const typename F::E (&x)[D],
+                                                         const typename F::E (&y)[D])
+{
+    constexpr int used = F::kWidenFree ? 0 : 1;
+    typename F::A s = f.widen(init);
+#pragma unroll
+    for (int mu = 0; mu < D; ++mu) {
+        if (mu + used >= F::kCap0 && ((mu + used - F::kCap0) % F::kCapR) == 0) s = f.relief(s);
         s = f.mad(x[mu], y[mu], s);
     }
     return s;

@@ -50,6 +50,9 @@ struct Fp31 {
     static constexpr int kCapR = 2;           // products an accumulator takes after relief()
     static constexpr bool kExact = true;
     static constexpr int kFieldId = 0;
+    // an accumulator that starts from widen(a) instead of zero still takes kCap0 products: a < 2^31 and
+    // 4 p (p-1) + 2^31 = 2^64 - 2^33 - 2^31 + 8, upper word < 2p
+    static constexpr bool kWidenFree = true;
 
     __device__ __forceinline__ Fp31(const Params&, int) {}
 
@@ -82,21 +85,19 @@ struct Fp31 {
         asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(lo), "r"(hi));
         return r;
     }
-    // canonical residue of any 64-bit accumulator: x = hi 2^32 + lo = 2 hi + lo (mod p) < 3*2^32,
-    // written in place -- add 2 hi to the whole accumulator (one IMAD.WIDE.U32), then take hi off
-    // the upper word (one IADD) -- so that no register pair has to be rebuilt around the low word;
-    // the word split / join is opaque inline PTX (register renaming only) so that the compiler
-    // cannot rewrite this back into "rebuild (lo, 0), then multiply-add"
+    // canonical residue of an accumulator whose upper word is < 2p (what the headroom rules guarantee):
+    // x = hi 2^32 + lo = 2 hi + (lo >> 31) + (lo & p) (mod p).  Five ALU instructions and one add, NO
+    // multiplier: the FMA-heavy pipe is the binding one (71 % busy at cfg2), and the fold by 2^32 = 2 as an
+    // IMAD.WIDE (rounds 1-2) spent 4 of its cycles per reduction, with both additions issued as IMAD.IADD
+    // on the same pipe on top.
     __device__ __forceinline__ E reduce(A x) const
     {
-        uint32_t lo, hi, tl, th;
+        uint32_t lo, hi;
         asm("mov.b64 {%0, %1}, %2;" : "=r"(lo), "=r"(hi) : "l"(x));
-        const A t0 = mad(hi, c_two32, x);
-        asm("mov.b64 {%0, %1}, %2;" : "=r"(tl), "=r"(th) : "l"(t0));
-        th -= hi;
-        A t;
-        asm("mov.b64 %0, {%1, %2};" : "=l"(t) : "r"(tl), "r"(th));
-        uint32_t r = (uint32_t)(t & kP) + (uint32_t)(t >> 31);    // < 2^31 + 6
+        hi = min(hi, hi - kP);                                    // < p
+        uint32_t s = __funnelshift_l(lo, hi, 1);                  // 2 hi + (lo >> 31) <= 2p - 1
+        s = min(s, s - kP);                                       // < p
+        const uint32_t r = (lo & kP) + s;                         // < 2p
         return min(r, r - kP);
     }
     __device__ __forceinline__ E neg(E a) const { return a ^ kP; }       // p - a, in [0,p]; 0 -> p
@@ -151,6 +152,7 @@ struct FpMont {
     static constexpr int kCapR = 2;
     static constexpr bool kExact = true;
     static constexpr int kFieldId = 2;
+    static constexpr bool kWidenFree = false;  // widen(a) = a R is a product like any other
     uint32_t p, pinv, r2, one_, half_;
 
     __device__ __forceinline__ FpMont(const Params& q, int i)
@@ -225,6 +227,7 @@ struct C128 {
     static constexpr int kCapR = 1 << 30;
     static constexpr bool kExact = false;
     static constexpr int kFieldId = 1;
+    static constexpr bool kWidenFree = true;
 
     __device__ __forceinline__ C128(const Params&, int) {}
 

@@ -260,7 +260,7 @@ struct TileSetup {
                     c = f.mul(c, z ? f.one() : s);
                 }
                 E u = f.inv(c);
-                u = f.dbl(f.dbl(u));
+                u = f.neg(f.dbl(f.dbl(u)));                                     // the table holds -1/P^2 (bg_unit.cuh)
                 int rl = vw + ((C::R - 1 - vw) / VW) * VW;                      // last r of this (half-)warp
                 if (vw >= C::R) rl = -1;
 #pragma unroll 1
@@ -275,7 +275,7 @@ struct TileSetup {
                 for (int r = vw; r < C::R; r += VW) {
                     const E s = Wt[r * TP];
                     if (f.is_zero(s)) status |= 1u;
-                    Wt[r * TP] = f.dbl(f.dbl(f.inv(s)));
+                    Wt[r * TP] = f.neg(f.dbl(f.dbl(f.inv(s))));
                 }
             }
             if (status_out && status) atomicOr(&t.stat[t.point], status);

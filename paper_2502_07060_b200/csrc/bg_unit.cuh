@@ -121,7 +121,7 @@ constexpr FlatProgram<N, W> make_flat_program()
 template <class F, int N, int D, int W, int S>
 __constant__ FlatProgram<N, W> c_flat_program = make_flat_program<F, N, D, W, S>();
 
-// the 4-gluon split (i..k | k+1..l | l+1..j): acc += 2 (A.C) J(k+1..l); na = -g A
+// the 4-gluon split (i..k | k+1..l | l+1..j): acc -= 2 (A.C) J(k+1..l); na = -g A
 template <class F, int D, int S>
 __device__ __forceinline__ void unit_quad(const F& f, const char* __restrict__ rb_, uint32_t bc,
                                           const typename F::E (&na)[D / S], typename F::A (&acc)[D / S])
@@ -131,19 +131,19 @@ __device__ __forceinline__ void unit_quad(const F& f, const char* __restrict__ r
     E bm[DL], c[DL];
     ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (bc & 0xffffu)), bm);
     ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (bc >> 16)), c);
-    const E cc = f.neg(f.dbl(lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, na, c)))));
+    const E ncc = f.dbl(lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, na, c))));       // -2 A.C
 #pragma unroll
-    for (int mu = 0; mu < DL; ++mu) acc[mu] = f.mad(cc, bm[mu], acc[mu]);
+    for (int mu = 0; mu < DL; ++mu) acc[mu] = f.mad(ncc, bm[mu], acc[mu]);
 }
 
-// one unit: the 3-gluon split (A | B) and its c4 4-gluon splits; entry and exit: every acc[] has room for
-// kCapR more products.  The 4-gluon splits are a run-time loop over pairs (the relief pattern of a pair is
+// one unit: the 3-gluon split (A | B) and its c4 4-gluon splits, SUBTRACTED from acc (nx2 = -2 covariant X,
+// nhsum = -sum_k h_k); entry and exit: every acc[] has room for kCapR more products.  The 4-gluon splits are a run-time loop over pairs (the relief pattern of a pair is
 // static), so there is ONE body for every c4 and the kernel stays inside the instruction cache for any n.
 template <class F, int MET, int N, int D, int S>
 __device__ __forceinline__ void unit_body(const F& f, int mu0, const typename F::E* __restrict__ rec,
                                           const typename F::E* __restrict__ sc, const FlatOp& o,
-                                          const uint32_t* __restrict__ quad, const typename F::E (&x2)[D / S],
-                                          typename F::A (&acc)[D / S], typename F::E& hsum)
+                                          const uint32_t* __restrict__ quad, const typename F::E (&nx2)[D / S],
+                                          typename F::A (&acc)[D / S], typename F::E& nhsum)
 {
     typedef typename F::E E;
     constexpr int DL = D / S, TP = 32 / S;
@@ -156,24 +156,28 @@ __device__ __forceinline__ void unit_body(const F& f, int mu0, const typename F:
     ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (o.pso & 0xffffu)), s);      // PS2_k, k = i+la-1
     const E ua = *reinterpret_cast<const E*>(sb_ + o.u), vb = *reinterpret_cast<const E*>(sb_ + o.v);
     lower_neg<F, MET, DL>(f, mu0, a, na);
-    const E h = f.neg(lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, na, b))));   // A.B
-    const E xa = lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, x2, a)));         // 2 X.A
-    const E xb = lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, x2, b)));         // 2 X.B
-    const E cb = f.sub(xa, ua);
-    const E ca = f.sub(vb, xb);
-    hsum = f.add(hsum, h);
+    const E nh = lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, na, b)));          // -A.B
+    E ncb, nca;                                                                        // U_A - 2X.A, 2X.B - V_B
+    if constexpr (S == 1) {
+        ncb = f.reduce(dot_plain_from<F, DL>(f, ua, nx2, a));
+        nca = f.neg(f.reduce(dot_plain_from<F, DL>(f, vb, nx2, b)));
+    } else {
+        ncb = f.add(ua, lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, nx2, a))));
+        nca = f.neg(f.add(vb, lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, nx2, b)))));
+    }
+    nhsum = f.add(nhsum, nh);
     auto relieve = [&]() {
 #pragma unroll
         for (int mu = 0; mu < DL; ++mu) acc[mu] = f.relief(acc[mu]);
     };
 #pragma unroll
     for (int mu = 0; mu < DL; ++mu) {
-        acc[mu] = f.mad(h, s[mu], acc[mu]);
-        acc[mu] = f.mad(cb, b[mu], acc[mu]);
+        acc[mu] = f.mad(nh, s[mu], acc[mu]);
+        acc[mu] = f.mad(ncb, b[mu], acc[mu]);
     }
     if (F::kExact) relieve();
 #pragma unroll
-    for (int mu = 0; mu < DL; ++mu) acc[mu] = f.mad(ca, a[mu], acc[mu]);      // room for one more product
+    for (int mu = 0; mu < DL; ++mu) acc[mu] = f.mad(nca, a[mu], acc[mu]);     // room for one more product
     const int c4 = o.qcf >> 16 & 0xffu;
     const uint32_t* qd = quad + (o.qcf & 0xffffu);
     int q = 0;
@@ -189,13 +193,14 @@ __device__ __forceinline__ void unit_body(const F& f, int mu0, const typename F:
     if (F::kExact) relieve();
 }
 
-// Finish the current whose bracket sum is in acc (room for kCapR more products): boundary term of the (P-Q)
-// sum, propagator, store, U and V; for the top current the amplitude instead (no propagator).
+// Finish the current whose bracket sum is in acc, NEGATED (room for kCapR more products): boundary term of the
+// (P-Q) sum, propagator (the table holds -1/P^2), store, U and V; for the top current the amplitude instead (no
+// propagator).  nx2 = -2 covariant P_{i,j}, nhsum = -sum_k h_k.
 template <class F, int MET, int N, int D, int W, int S, bool KW>
 __device__ __forceinline__ void unit_finish(const F& f, const TileLane<F, N, D, W, S, KW>& t, typename F::E* rec,
                                             typename F::E* sc, const FlatOp& o, bool top,
-                                            const typename F::E (&x2)[D / S], typename F::A (&acc)[D / S],
-                                            typename F::E hsum, typename F::E* out, typename F::E* currents)
+                                            const typename F::E (&nx2)[D / S], typename F::A (&acc)[D / S],
+                                            typename F::E nhsum, typename F::E* out, typename F::E* currents)
 {
     typedef TileCfg<F, N, D, W, S, KW> C;
     typedef typename F::E E;
@@ -204,7 +209,7 @@ __device__ __forceinline__ void unit_finish(const F& f, const TileLane<F, N, D, 
     E l[DL], h[DL];
     ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (o.lh & 0xffffu)), l);     // PS2_{i-1}
     ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (o.lh >> 16)), h);         // PS2_j
-    const E nhh = f.neg(f.mul(hsum, f.half()));                 // -(sum_k h_k)/2
+    const E nhh = f.neg(f.mul(nhsum, f.half()));                // +(sum_k h_k)/2: minus the boundary coefficient
     if constexpr (F::kExact) {
         // one product per component: the two ALU instructions of the add are cheaper than a
         // second IMAD.WIDE (the multiplier pipe is the binding one)
@@ -220,26 +225,31 @@ __device__ __forceinline__ void unit_finish(const F& f, const TileLane<F, N, D, 
     E v[DL];
     if (!top) {
         const uint32_t own = o.pso >> 16, urow = o.w >> 8 & 0xffu;
-        const E w = sc[(C::SC_W + urow - N) * TP];              // 1/P^2
+        const E w = sc[(C::SC_W + urow - N) * TP];              // -1/P^2
 #pragma unroll
         for (int mu = 0; mu < DL; ++mu) v[mu] = f.mul(f.reduce(acc[mu]), w);
         st_vec<F, DL>(reinterpret_cast<E*>(rb_ + own), v);
-        const E c2 = lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, x2, v)));    // 2 P_{i,j} . J(i..j)
-        sc[(C::SC_U + urow) * TP] = f.add(c2, hsum);
-        sc[(C::SC_V + urow - N) * TP] = f.sub(c2, hsum);
+        const E nc2 = lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, nx2, v)));  // -2 P_{i,j} . J(i..j)
+        sc[(C::SC_U + urow) * TP] = f.canon(f.neg(f.add(nc2, nhsum)));               // U = 2 P.J + sum_k h_k
+        sc[(C::SC_V + urow - N) * TP] = f.sub(nhsum, nc2);                           // V = 2 P.J - sum_k h_k
+        if (currents && t.live) {
+            E* dst = currents + (t.pt * M * M + (long long)(o.w & 0xffu)) * D + t.mu0;
+#pragma unroll
+            for (int mu = 0; mu < DL; ++mu) dst[mu] = f.to_output(v[mu]);
+        }
     } else {
 #pragma unroll
         for (int mu = 0; mu < DL; ++mu) v[mu] = f.reduce(acc[mu]);
         E e[DL], ne[DL];
         ld_vec<F, DL>(rec + (N - 1) * D, e);
         lower_neg<F, MET, DL>(f, t.mu0, e, ne);
-        const E nout = lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, ne, v)));  // -(eps_n . N)
-        if (t.live && t.half == 0) *out = f.to_output(f.neg(nout));
-    }
-    if (currents && t.live) {
-        E* dst = currents + (t.pt * M * M + (long long)(o.w & 0xffu)) * D + t.mu0;
+        const E o_ = lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, ne, v)));    // -(eps_n . v) = eps_n . N
+        if (t.live && t.half == 0) *out = f.to_output(o_);
+        if (currents && t.live) {                               // v = -N(1..m)
+            E* dst = currents + (t.pt * M * M + (long long)(o.w & 0xffu)) * D + t.mu0;
 #pragma unroll
-        for (int mu = 0; mu < DL; ++mu) dst[mu] = f.to_output(v[mu]);
+            for (int mu = 0; mu < DL; ++mu) dst[mu] = f.to_output(f.neg(v[mu]));
+        }
     }
 }
 
@@ -258,11 +268,11 @@ __device__ __forceinline__ void unit_sweep_body(const F& f, const TileLane<F, N,
     char* rb_ = reinterpret_cast<char*>(rec);
     char* sb_ = reinterpret_cast<char*>(sc);
     uint32_t* flags = t.stat + TP + (threadIdx.x & 31);         // this lane's parked flags, [slot * 32]
-    E x2[DL];
+    E nx2[DL];
     A acc[DL];
-    E hsum = f.ezero();
+    E nhsum = f.ezero();
 #pragma unroll
-    for (int mu = 0; mu < DL; ++mu) { x2[mu] = f.ezero(); acc[mu] = f.zero(); }
+    for (int mu = 0; mu < DL; ++mu) { nx2[mu] = f.ezero(); acc[mu] = f.zero(); }
     const int k0 = fp.beg[warp], k1 = fp.beg[warp + 1];
 #pragma unroll 1
     for (int k = k0; k < k1; ++k) {
@@ -272,12 +282,12 @@ __device__ __forceinline__ void unit_sweep_body(const F& f, const TileLane<F, N,
             E l[DL], h[DL];
             ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (o.lh & 0xffffu)), l);     // PS2_{i-1}
             ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (o.lh >> 16)), h);         // PS2_j
-            lower_diff<F, MET, DL>(f, t.mu0, h, l, x2);                               // 2 * covariant P_{i,j}
+            lower_diff<F, MET, DL>(f, t.mu0, l, h, nx2);                              // -2 * covariant P_{i,j}
 #pragma unroll
             for (int mu = 0; mu < DL; ++mu) acc[mu] = f.zero();
-            hsum = f.ezero();
+            nhsum = f.ezero();
         }
-        if (fl & OP_UNIT) unit_body<F, MET, N, D, S>(f, t.mu0, rec, sc, o, fp.quad, x2, acc, hsum);
+        if (fl & OP_UNIT) unit_body<F, MET, N, D, S>(f, t.mu0, rec, sc, o, fp.quad, nx2, acc, nhsum);
         if (fl & OP_PART) {
             // a later part of a current shared between warps: park the partial sums, tell the finisher.
             // (a byte offset from the table, not slot * (D + 1): a run-time multiply here makes ptxas give up the
@@ -285,7 +295,7 @@ __device__ __forceinline__ void unit_sweep_body(const F& f, const TileLane<F, N,
             E* scr = reinterpret_cast<E*>(sb_ + C::SC_SCR * TP * (int)sizeof(E) + o.aux);
 #pragma unroll
             for (int mu = 0; mu < DL; ++mu) scr[(t.mu0 + mu) * TP] = f.reduce(acc[mu]);
-            scr[D * TP] = hsum;
+            scr[D * TP] = nhsum;
             // the lane that reads a parked value is this lane of the finishing warp: a per-lane flag, raised after
             // the values (fence), tells it that they are there; `epoch` is unique per sweep and level
             __threadfence_block();
@@ -310,13 +320,13 @@ __device__ __forceinline__ void unit_sweep_body(const F& f, const TileLane<F, N,
                 const E* scr = sc + (C::SC_SCR + slot * (D + 1)) * TP;
 #pragma unroll
                 for (int mu = 0; mu < DL; ++mu) sum[mu] = f.add(sum[mu], scr[(t.mu0 + mu) * TP]);
-                hsum = f.add(hsum, scr[D * TP]);
+                nhsum = f.add(nhsum, scr[D * TP]);
             }
 #pragma unroll
             for (int mu = 0; mu < DL; ++mu) acc[mu] = f.addw(acc[mu], sum[mu]);   // one of the kCapR products of room
         }
         if (fl & OP_FIN)
-            unit_finish<F, MET, N, D, W, S, KW>(f, t, rec, sc, o, (fl & OP_TOP) != 0, x2, acc, hsum, out, currents);
+            unit_finish<F, MET, N, D, W, S, KW>(f, t, rec, sc, o, (fl & OP_TOP) != 0, nx2, acc, nhsum, out, currents);
         if (fl & OP_LEND) __syncthreads();
     }
 }
