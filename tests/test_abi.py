@@ -102,3 +102,23 @@ def test_product_does_not_import_the_oracle():
 def test_compile_time_schedules_are_valid(lib):
     """every splitting of every current exactly once, parts gathered once, barriers by every warp"""
     assert binding.bg_selftest_schedules() == 0
+
+
+def test_headline_kernel_keeps_the_uniform_datapath(lib):
+    """The sweep of the tiled kernel is a run-time loop over a table in constant memory: its control flow and
+    table loads must sit on the uniform datapath (BRA.U / ULOP3 / LDCU).  ptxas drops that silently for innocent
+    looking source changes (a run-time multiply on a table field, a named barrier, a select on a table flag:
+    +4 % to +18 % at cfg2), so the SASS of the default instances is checked here."""
+    import shutil
+    import subprocess
+    obj = os.path.join(build.CSRC, "bg_inst_default.o")
+    tool = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(obj) or not os.path.exists(tool):
+        pytest.skip("no object file / cuobjdump")
+    sass = subprocess.run([tool, "-sass", obj], capture_output=True, text=True, check=True).stdout
+    kernels = re.split(r"\n\s*Function : ", sass)[1:]
+    plain = [k for k in kernels if k.startswith("_ZN2bg14bg_unit_kernel") and "ELb0EEE" in k.split("\n", 1)[0]]
+    assert plain, "no tiled kernel in the default table"
+    for k in plain:
+        name = k.split("\n", 1)[0]
+        assert k.count("BRA.U") >= 5 and k.count("LDCU") >= 3, name
