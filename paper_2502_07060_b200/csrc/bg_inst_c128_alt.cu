@@ -8,4 +8,5 @@ BG_DEFINE_TABLE(c128_alt,
     unit_entry<C128, MM, 6, 4, 4, 1>(),
     unit_entry<C128, MM, 12, 6, 8, 2>(),
     unit_entry<C128, MM, 12, 6, 4, 2>(),
+    unit_entry<C128, MM, 12, 6, 16, 2>(),
 )

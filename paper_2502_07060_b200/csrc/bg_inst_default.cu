@@ -8,5 +8,5 @@ BG_DEFINE_TABLE(default,
     unit_entry<Fp31, MM, 10, 8, 8>(),         // cfg3
     unit_entry<Fp31, MM, 12, 6, 8>(),         // cfg4a
     reg_entry<C128, MM, 6, 4>(),              // cfg1
-    unit_entry<C128, MM, 12, 6, 16, 2>(),     // cfg4b (W = 16: 0.861 ms, W = 8: 0.901 ms)
+    unit_entry<C128, MM, 12, 6, 12, 2>(),     // cfg4b (W = 8 / 12 / 14 / 16: 0.884 / 0.828 / 0.843 / 0.842 ms)
 )

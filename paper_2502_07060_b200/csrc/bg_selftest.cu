@@ -101,5 +101,8 @@ extern "C" int bg_selftest_schedules(void)
     if ((rc = check_level_program<12, 4>())) return rc - 170000;
     if ((rc = check_level_program<16, 8>())) return rc - 180000;
     if ((rc = check_level_program<11, 8>())) return rc - 190000;
+    if ((rc = check_level_program<12, 12>())) return rc - 200000;
+    if ((rc = check_level_program<8, 3>())) return rc - 210000;
+    if ((rc = check_level_program<16, 16>())) return rc - 220000;
     return rc;
 }
