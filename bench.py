@@ -505,11 +505,21 @@ def run_gpu(args) -> None:
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    # BG_BENCH_SMOKE_SHARED_DEVICE=1: a code-path smoke test of the N > 1 branch on a box with fewer GPUs than
+    # ranks (ranks share devices, rendezvous and reductions over gloo).  The ranks are independent -- no kernel
+    # waits on another rank -- but the line is marked "shared_device" and is NOT a scaling measurement.
+    shared = os.environ.get("BG_BENCH_SMOKE_SHARED_DEVICE") == "1" and local >= torch.cuda.device_count()
+    if shared:
+        local = local % torch.cuda.device_count()
+    shared = shared or (os.environ.get("BG_BENCH_SMOKE_SHARED_DEVICE") == "1" and world > torch.cuda.device_count())
     torch.cuda.set_device(local)
     dist = None
     if world > 1:
         import torch.distributed as dist_mod
-        dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if shared:
+            dist_mod.init_process_group("gloo")
+        else:
+            dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local))
         dist = dist_mod
     from paper_2502_07060_b200 import binding, measure, sharding
     binding.load()
@@ -525,7 +535,8 @@ def run_gpu(args) -> None:
     with ClockSampler(nvml_index) as clk:
         res = device_bench(binding, torch, name, batch, start, args.steps, args.warmup, dist)
     clocks = clk.summary()
-    total_ms = torch.tensor([res["total_ms"]], dtype=torch.float64, device="cuda")
+    red_dev = "cpu" if shared else "cuda"                 # gloo reduces host tensors
+    total_ms = torch.tensor([res["total_ms"]], dtype=torch.float64, device=red_dev)
     if dist is not None:
         dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
     total_ms = float(total_ms.item())
@@ -536,7 +547,7 @@ def run_gpu(args) -> None:
     # end to end through the host entry point
     e2e_steps = max(3, min(args.steps, args.e2e_steps))
     e2e = e2e_bench(binding, torch, name, res["mom"], res["pol"], e2e_steps, min(args.warmup, 3), dist)
-    e2e_t = torch.tensor([e2e["s_per_step"]], dtype=torch.float64, device="cuda")
+    e2e_t = torch.tensor([e2e["s_per_step"]], dtype=torch.float64, device=red_dev)
     if dist is not None:
         dist.all_reduce(e2e_t, op=dist.ReduceOp.MAX)
     e2e_value = world * batch / float(e2e_t.item())
@@ -558,6 +569,8 @@ def run_gpu(args) -> None:
                 "steps": e2e_steps, "matches_device_path": same,
                 "api": "bg_amplitudes_host (pinned host buffers, chunked H2D/kernel/D2H pipeline)"},
         "gpu_launches": args.steps,
+        **({"shared_device": "SMOKE TEST of the N > 1 code path: the ranks shared GPUs; not a scaling number"}
+           if shared else {}),
         "clocks": clocks,
         "kernel": binding.bg_kernel_info(binding.FIELD_FP31 if cfg["field"] == "fp31" else binding.FIELD_C128,
                                          cfg["n"], cfg["d"]),
