@@ -23,6 +23,7 @@ namespace bg {
 // byte offset from the lane's record / scalar base, so the sweep is a single run-time loop whose body needs
 // two 16-byte constant loads and a few warp-uniform flag tests (round 2 decoded a task word, a unit-table
 // entry and a level header per iteration: 4.2 k of the 20.3 k instructions per cfg2 tile).
+constexpr uint32_t OP_PAIR = 1u;      // this unit and the next one belong to the same task (see unit_pair_body)
 constexpr uint32_t OP_START = 2u;     // first op of a task: form 2 P_{i,j}, clear the bracket sums
 constexpr uint32_t OP_UNIT = 4u;      // a 3-gluon split with its c4 4-gluon splits
 constexpr uint32_t OP_PART = 8u;      // last op of a later part of a shared current: park the partial sums, raise the flag
@@ -103,7 +104,8 @@ constexpr FlatProgram<N, W> make_flat_program()
                     o.w = wfield;
                     o.lh = lh;
                     o.aux = aux;
-                    const uint32_t fl = OP_UNIT | (la == lo + 1 ? OP_START : 0u) | (la == hi ? endf : 0u);
+                    const uint32_t fl = OP_UNIT | (la == lo + 1 ? OP_START : 0u) | (la == hi ? endf : 0u) |
+                                        ((la - lo) % 2 == 1 && la < hi ? OP_PAIR : 0u);
                     o.qcf = (uint32_t)nq | (uint32_t)c4 << 16 | fl << 24;
                     for (int lb = 1; lb <= c4; ++lb)
                         f.quad[nq++] = (uint32_t)((lv_rowbase<N>(lb) + ci + la) * RB) |
@@ -136,21 +138,18 @@ __device__ __forceinline__ void unit_quad(const F& f, const char* __restrict__ r
     for (int mu = 0; mu < DL; ++mu) acc[mu] = f.mad(ncc, bm[mu], acc[mu]);
 }
 
-// one unit: the 3-gluon split (A | B) and its c4 4-gluon splits, SUBTRACTED from acc (nx2 = -2 covariant X,
-// nhsum = -sum_k h_k); entry and exit: every acc[] has room for kCapR more products.  The 4-gluon splits are a run-time loop over pairs (the relief pattern of a pair is
-// static), so there is ONE body for every c4 and the kernel stays inside the instruction cache for any n.
-template <class F, int MET, int N, int D, int S>
-__device__ __forceinline__ void unit_body(const F& f, int mu0, const typename F::E* __restrict__ rec,
-                                          const typename F::E* __restrict__ sc, const FlatOp& o,
-                                          const uint32_t* __restrict__ quad, const typename F::E (&nx2)[D / S],
-                                          typename F::A (&acc)[D / S], typename F::E& nhsum)
+// the 3-gluon split (A | B) of a unit, SUBTRACTED from acc (nx2 = -2 covariant X, nhsum = -sum_k h_k); returns
+// na = -g A for the unit's 4-gluon splits.  Entry: room for kCapR products; exit: room for one more.
+template <class F, int MET, int D, int S>
+__device__ __forceinline__ void unit_split3(const F& f, int mu0, const char* __restrict__ rb_,
+                                            const char* __restrict__ sb_, const FlatOp& o,
+                                            const typename F::E (&nx2)[D / S], typename F::A (&acc)[D / S],
+                                            typename F::E& nhsum, typename F::E (&na)[D / S])
 {
     typedef typename F::E E;
     constexpr int DL = D / S, TP = 32 / S;
-    static_assert(F::kCapR >= 2, "the relief pattern below assumes room for two products after relief()");
-    const char* rb_ = reinterpret_cast<const char*>(rec);
-    const char* sb_ = reinterpret_cast<const char*>(sc);
-    E a[DL], b[DL], s[DL], na[DL];
+    static_assert(F::kCapR >= 2, "the relief pattern assumes room for two products after relief()");
+    E a[DL], b[DL], s[DL];
     ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (o.ab & 0xffffu)), a);
     ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (o.ab >> 16)), b);
     ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (o.pso & 0xffffu)), s);      // PS2_k, k = i+la-1
@@ -166,18 +165,38 @@ __device__ __forceinline__ void unit_body(const F& f, int mu0, const typename F:
         nca = f.neg(f.add(vb, lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, nx2, b)))));
     }
     nhsum = f.add(nhsum, nh);
-    auto relieve = [&]() {
-#pragma unroll
-        for (int mu = 0; mu < DL; ++mu) acc[mu] = f.relief(acc[mu]);
-    };
 #pragma unroll
     for (int mu = 0; mu < DL; ++mu) {
         acc[mu] = f.mad(nh, s[mu], acc[mu]);
         acc[mu] = f.mad(ncb, b[mu], acc[mu]);
     }
-    if (F::kExact) relieve();
+    if (F::kExact) {
+#pragma unroll
+        for (int mu = 0; mu < DL; ++mu) acc[mu] = f.relief(acc[mu]);
+    }
 #pragma unroll
     for (int mu = 0; mu < DL; ++mu) acc[mu] = f.mad(nca, a[mu], acc[mu]);     // room for one more product
+}
+
+// one unit: the 3-gluon split (A | B) and its c4 4-gluon splits; entry and exit: every acc[] has room for kCapR
+// more products.  The 4-gluon splits are a run-time loop over pairs (the relief pattern of a pair is static), so
+// there is ONE body for every c4 and the kernel stays inside the instruction cache for any n.
+template <class F, int MET, int N, int D, int S>
+__device__ __forceinline__ void unit_body(const F& f, int mu0, const typename F::E* __restrict__ rec,
+                                          const typename F::E* __restrict__ sc, const FlatOp& o,
+                                          const uint32_t* __restrict__ quad, const typename F::E (&nx2)[D / S],
+                                          typename F::A (&acc)[D / S], typename F::E& nhsum)
+{
+    typedef typename F::E E;
+    constexpr int DL = D / S;
+    const char* rb_ = reinterpret_cast<const char*>(rec);
+    const char* sb_ = reinterpret_cast<const char*>(sc);
+    E na[DL];
+    unit_split3<F, MET, D, S>(f, mu0, rb_, sb_, o, nx2, acc, nhsum, na);
+    auto relieve = [&]() {
+#pragma unroll
+        for (int mu = 0; mu < DL; ++mu) acc[mu] = f.relief(acc[mu]);
+    };
     const int c4 = o.qcf >> 16 & 0xffu;
     const uint32_t* qd = quad + (o.qcf & 0xffffu);
     int q = 0;
@@ -191,6 +210,54 @@ __device__ __forceinline__ void unit_body(const F& f, int mu0, const typename F:
         unit_quad<F, D, S>(f, rb_, qd[q], na, acc);
     }
     if (F::kExact) relieve();
+}
+
+// Two consecutive units (i..k | ..) and (i..k+1 | ..) of one current together: their 4-gluon splits with the same
+// right factor C = J(l+1..j) share ONE load of C (the 4-gluon split q >= 1 of the first unit and q - 1 of the second),
+// 1.5 instead of 2 vector loads per split.  Used where shared-memory traffic binds (complex128: a 16-byte element
+// per lane makes every vector load 4 wavefronts per warp); same arithmetic, other order of the sums.
+template <class F, int MET, int N, int D, int S>
+__device__ __forceinline__ void unit_pair_body(const F& f, int mu0, const typename F::E* __restrict__ rec,
+                                               const typename F::E* __restrict__ sc, const FlatOp& o1,
+                                               const FlatOp& o2, const uint32_t* __restrict__ quad,
+                                               const typename F::E (&nx2)[D / S], typename F::A (&acc)[D / S],
+                                               typename F::E& nhsum)
+{
+    typedef typename F::E E;
+    constexpr int DL = D / S, TP = 32 / S;
+    const char* rb_ = reinterpret_cast<const char*>(rec);
+    const char* sb_ = reinterpret_cast<const char*>(sc);
+    auto relieve = [&]() {
+        if (F::kExact) {
+#pragma unroll
+            for (int mu = 0; mu < DL; ++mu) acc[mu] = f.relief(acc[mu]);
+        }
+    };
+    E na1[DL], na2[DL];
+    unit_split3<F, MET, D, S>(f, mu0, rb_, sb_, o1, nx2, acc, nhsum, na1);
+    relieve();
+    unit_split3<F, MET, D, S>(f, mu0, rb_, sb_, o2, nx2, acc, nhsum, na2);
+    const int c4 = o1.qcf >> 16 & 0xffu;                       // the second unit has c4 - 1
+    const uint32_t* qd1 = quad + (o1.qcf & 0xffffu);
+    const uint32_t* qd2 = quad + (o2.qcf & 0xffffu);
+    if (c4 > 0) unit_quad<F, D, S>(f, rb_, qd1[0], na1, acc);   // (k+1 | k+2..j): no partner
+    relieve();
+#pragma unroll 1
+    for (int q = 1; q < c4; ++q) {
+        const uint32_t bc1 = qd1[q], bc2 = qd2[q - 1];
+        E c[DL], m1[DL], m2[DL];
+        ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (bc1 >> 16)), c);
+        ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (bc1 & 0xffffu)), m1);
+        ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (bc2 & 0xffffu)), m2);
+        const E n1 = f.dbl(lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, na1, c))));    // -2 A1.C
+        const E n2 = f.dbl(lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, na2, c))));    // -2 A2.C
+#pragma unroll
+        for (int mu = 0; mu < DL; ++mu) {
+            acc[mu] = f.mad(n1, m1[mu], acc[mu]);
+            acc[mu] = f.mad(n2, m2[mu], acc[mu]);
+        }
+        relieve();
+    }
 }
 
 // Finish the current whose bracket sum is in acc, NEGATED (room for kCapR more products): boundary term of the
@@ -262,6 +329,7 @@ __device__ __forceinline__ void unit_sweep_body(const F& f, const TileLane<F, N,
     typedef typename F::E E;
     typedef typename F::A A;
     constexpr int DL = C::DL, TP = C::TP;
+    constexpr bool kPairs = !F::kExact;                         // unit pairs where shared-memory traffic binds
     const FlatProgram<N, W>& fp = c_flat_program<F, N, D, W, S>;
     E* rec = t.rec();
     E* sc = t.sc();
@@ -287,30 +355,41 @@ __device__ __forceinline__ void unit_sweep_body(const F& f, const TileLane<F, N,
             for (int mu = 0; mu < DL; ++mu) acc[mu] = f.zero();
             nhsum = f.ezero();
         }
-        if (fl & OP_UNIT) unit_body<F, MET, N, D, S>(f, t.mu0, rec, sc, o, fp.quad, nx2, acc, nhsum);
-        if (fl & OP_PART) {
+        if constexpr (kPairs) {
+            if (fl & OP_PAIR) {
+                unit_pair_body<F, MET, N, D, S>(f, t.mu0, rec, sc, fp.op[k], fp.op[k + 1], fp.quad, nx2, acc, nhsum);
+                ++k;                                            // the second unit carries the task's end flags
+            } else if (fl & OP_UNIT) {
+                unit_body<F, MET, N, D, S>(f, t.mu0, rec, sc, fp.op[k], fp.quad, nx2, acc, nhsum);
+            }
+        } else if (fl & OP_UNIT) {
+            unit_body<F, MET, N, D, S>(f, t.mu0, rec, sc, fp.op[k], fp.quad, nx2, acc, nhsum);
+        }
+        const FlatOp& oe = fp.op[k];                           // the op that carries the task's end flags
+        const uint32_t fle = oe.qcf >> 24;
+        if (fle & OP_PART) {
             // a later part of a current shared between warps: park the partial sums, tell the finisher.
             // (a byte offset from the table, not slot * (D + 1): a run-time multiply here makes ptxas give up the
             // uniform datapath for the whole sweep, +4.5 % at cfg2)
-            E* scr = reinterpret_cast<E*>(sb_ + C::SC_SCR * TP * (int)sizeof(E) + o.aux);
+            E* scr = reinterpret_cast<E*>(sb_ + C::SC_SCR * TP * (int)sizeof(E) + oe.aux);
 #pragma unroll
             for (int mu = 0; mu < DL; ++mu) scr[(t.mu0 + mu) * TP] = f.reduce(acc[mu]);
             scr[D * TP] = nhsum;
             // the lane that reads a parked value is this lane of the finishing warp: a per-lane flag, raised after
             // the values (fence), tells it that they are there; `epoch` is unique per sweep and level
             __threadfence_block();
-            *reinterpret_cast<volatile uint32_t*>(flags + (o.w >> 20)) = epoch0 + (o.w >> 16 & 15u);
+            *reinterpret_cast<volatile uint32_t*>(flags + (oe.w >> 20)) = epoch0 + (oe.w >> 16 & 15u);
         }
-        if (fl & OP_GATHER) {
+        if (fle & OP_GATHER) {
             // the finisher (owner of the first units, this is its last task of the level): the other parts were
             // first tasks of their warps and are parked by now
-            const uint32_t epoch = epoch0 + (o.w >> 16 & 15u);
-            for (uint32_t m2 = o.aux; m2; m2 &= m2 - 1) {
+            const uint32_t epoch = epoch0 + (oe.w >> 16 & 15u);
+            for (uint32_t m2 = oe.aux; m2; m2 &= m2 - 1) {
                 const volatile uint32_t* fl_ = flags + 32 * (__ffs(m2) - 1);
                 while (!__all_sync(0xffffffffu, *fl_ == epoch)) {}    // warp-uniform exit
             }
             __threadfence_block();
-            uint32_t mask = o.aux;
+            uint32_t mask = oe.aux;
             E sum[DL];
 #pragma unroll
             for (int mu = 0; mu < DL; ++mu) sum[mu] = f.ezero();
@@ -325,9 +404,9 @@ __device__ __forceinline__ void unit_sweep_body(const F& f, const TileLane<F, N,
 #pragma unroll
             for (int mu = 0; mu < DL; ++mu) acc[mu] = f.addw(acc[mu], sum[mu]);   // one of the kCapR products of room
         }
-        if (fl & OP_FIN)
-            unit_finish<F, MET, N, D, W, S, KW>(f, t, rec, sc, o, (fl & OP_TOP) != 0, nx2, acc, nhsum, out, currents);
-        if (fl & OP_LEND) __syncthreads();
+        if (fle & OP_FIN)
+            unit_finish<F, MET, N, D, W, S, KW>(f, t, rec, sc, oe, (fle & OP_TOP) != 0, nx2, acc, nhsum, out, currents);
+        if (fle & OP_LEND) __syncthreads();
     }
 }
 
