@@ -100,7 +100,7 @@ def test_product_does_not_import_the_oracle():
 
 
 def test_compile_time_schedules_are_valid(lib):
-    """every splitting of every current exactly once, parts gathered once, barriers by every warp"""
+    """every splitting of every current exactly once, shared currents handed over consistently"""
     assert binding.bg_selftest_schedules() == 0
 
 
