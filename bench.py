@@ -19,7 +19,7 @@ it stands, on this box's host cores, on a bounded sample), `e2e` (the same metri
 `clocks`, `gpu_launches`, `per_config` (short device-resident timings of the other BASELINE.json
 configs, each with its own oracle timing and, for complex128, the branch statistics of tolerance
 rule R9), `features` (the SURVEY.md 8(f) rows: state configurations, generic prime, alternating
-metric, colour orderings, state sum, device generator and states, the general kernel) and
+metric, colour orderings, state sum, device generator and states, shapes without a compiled instance) and
 `e2e_seeded` (seed -> amplitudes on the host with the generator on the device); N=1 only,
 `--headline-only` skips them.
 `--impl reference` times the CPU oracle alone (this tier's reference arm).
@@ -377,14 +377,14 @@ def run_features(binding, torch, steps: int) -> list:
     pb = B.problem(B.FIELD_FP31, n, d, n_orderings=K, orderings_ptr=dperm.data_ptr())
     row(f"f4 colour orderings: n=8 d=6 F_p, 2^15 points x K={K}", bo * K,
         time_device(torch, lambda: ev(pb, bo, mom, pol, outk), steps))
-    # the general kernel (shapes outside the compiled grid): the performance cliff bg.h documents
+    # shapes outside the compiled grid: the tiled kernel with a run-time n (bg_rt_kernel)
     for (gn, gd, gb) in ((13, 5, 1 << 15), (16, 4, 1 << 14)):
         mom, pol, _ = B.generate(B.FIELD_FP31, gn, gd, gb, seed=0)
         outg = torch.empty(gb, dtype=torch.int32, device="cuda")
         pb = B.problem(B.FIELD_FP31, gn, gd)
         ms = time_device(torch, lambda: ev(pb, gb, mom, pol, outg), max(3, steps // 4))
         oc = op_counts("fp31", gn, gd)
-        row(f"general kernel: n={gn} d={gd} F_p, {gb} points", gb, ms,
+        row(f"uncompiled shape (run-time-n tiled kernel): n={gn} d={gd} F_p, {gb} points", gb, ms,
             roofline_frac=oc["mul_ref"] * gb / (ms * 1e-3) / (SM_COUNT * WIDE_MUL_LANES_PER_CLK_PER_SM * 1.965e9),
             kernel=B.bg_kernel_info(B.FIELD_FP31, gn, gd))
     # Eq.(4) state sum: HBM-bound

@@ -38,13 +38,16 @@
  *   limits    4 <= n <= 16, 4 <= d <= 16 (the paper validates d = 4..10).
  *   memory    the caller owns every buffer; DEVICE pointers unless the name says host.
  *             Device pointers must be 16-byte aligned; out must not alias the inputs.
- *             The library allocates no device memory and keeps no per-call state.
+ *             The library keeps no per-call state and allocates no device memory, with one exception:
+ *             the first call for a shape (n, d) that has no compiled instance copies the work
+ *             schedule of that shape to the device it runs on (a few KB per shape and device, built
+ *             on the host, kept for the life of the process; that first call is synchronous).
  *   stream    launches are asynchronous on `stream`; nothing synchronises.
  *   errors    return value: BG_OK or a negative bg_status_t; nothing is thrown, nothing
  *             aborts.  Arguments are checked on the host before any launch.  batch == 0 is
  *             a no-op returning BG_OK.
  *   tuning    bg_set_kernel_override() restricts the kernel selection for A/B measurements (it never
- *             changes results); the environment variables BG_KERNEL = unit1 | unit2 | reg | general and
+ *             changes results); the environment variables BG_KERNEL = unit1 | unit2 | reg | rt | general and
  *             BG_KERNEL_W = <warps per tile> give its initial value, read ONCE when the library is loaded.
  *             Without either (the normal case) the default instance of the shape is launched.
  *   1/0       inv(0) := 0 in both fields (what Fermat's a^(p-2) gives); a point where some
@@ -215,9 +218,12 @@ int bg_op_count(int field, int n, int d, bg_opcount_t* out);
 
 /* Launch configuration the library would use for (field, n, d). */
 typedef struct {
-    int specialised;         /* 0: bg_general_kernel (run-time n, one thread per point); (n, d) compiled in:
-                                1 bg_unit_kernel with one lane per point, 2 bg_unit_kernel with two lanes per
-                                point, 3 bg_reg_kernel (currents in registers) -- the one a call would launch */
+    int specialised;         /* (n, d) compiled in: 1 bg_unit_kernel with one lane per point, 2 bg_unit_kernel with
+                                two lanes per point, 3 bg_reg_kernel (currents in registers); any other shape:
+                                4 bg_rt_kernel (the tiled kernel with a run-time n and a host-built schedule; one
+                                state configuration, one ordering), 0 bg_general_kernel (one thread per point:
+                                several state configurations / orderings on an uncompiled shape, and records too
+                                large for a 16-point tile) -- the one a call would launch */
     int threads_per_block;
     int points_per_block;
     int smem_bytes_per_block;
@@ -229,8 +235,8 @@ int bg_kernel_info(int field, int n, int d, bg_kernel_info_t* out);             
 int bg_kernel_info_problem(const bg_problem_t* problem, bg_kernel_info_t* out);
 
 /* Restrict the kernel selection of all later calls (process-wide; for A/B measurements, not meant to
- * be changed while other threads are inside the library).  kind: -1 default, 1 / 2 / 3 as in
- * bg_kernel_info_t.specialised, 0 the general kernel; warps: warps per tile, 0 = the first instance
+ * be changed while other threads are inside the library).  kind: -1 default, 1 / 2 / 3 / 4 as in
+ * bg_kernel_info_t.specialised (4 also on compiled shapes), 0 the general kernel; warps: warps per tile, 0 = the first instance
  * of that kind.  A shape with no matching instance falls back to its default.  Returns BG_OK. */
 int bg_set_kernel_override(int kind, int warps);
 

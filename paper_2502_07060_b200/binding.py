@@ -19,7 +19,7 @@ from . import build as _build
 FIELD_FP31, FIELD_C128, FIELD_FPMONT = 0, 1, 2
 METRIC_MOSTLY_MINUS, METRIC_ALTERNATING = 0, 1
 MAX_PRIMES = 8
-KERNEL_KINDS = {"default": -1, "general": 0, "unit1": 1, "unit2": 2, "reg": 3}
+KERNEL_KINDS = {"default": -1, "general": 0, "unit1": 1, "unit2": 2, "reg": 3, "rt": 4}
 BG_OK, BG_ERR_ARG, BG_ERR_UNSUPPORTED, BG_ERR_CUDA = 0, -1, -2, -3
 PEAK_KINDS = {"imad_wide": 0, "imad": 1, "alu": 2, "mix": 3, "modmul": 4, "dfma": 5,
               "lds32": 6, "lds64": 7, "lds128": 8, "mix2": 9, "mix3": 10, "imad_wide_rz": 11}
@@ -183,7 +183,7 @@ def bg_generate(field, prime, metric, n, d, batch, seed, start, helicities, mome
 
 
 def bg_set_kernel_override(kind=-1, warps=0):
-    """kind: -1 / "default", or "general", "unit1", "unit2", "reg" (bg.h)"""
+    """kind: -1 / "default", or "general", "unit1", "unit2", "reg", "rt" (bg.h)"""
     return load().bg_set_kernel_override(KERNEL_KINDS[kind] if isinstance(kind, str) else kind, warps)
 
 

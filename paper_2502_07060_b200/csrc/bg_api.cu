@@ -13,6 +13,7 @@
 #include "bg_entries.h"
 #include "bg_general.cuh"     // GeneralLayout (host side of the record layout)
 #include "bg_host_util.h"
+#include "bg_rt_host.h"
 
 namespace {
 
@@ -37,6 +38,11 @@ struct Launch {
     int smem = 0;
     int stride = 0;                    // general kernel: record stride in elements
     std::atomic<uint64_t> attr_done{0};   // bit i: cudaFuncSetAttribute done on device i
+    // bg_rt_kernel: layout and schedule built by the host (kept for the life of the process), and the copy of
+    // the tables on every device the shape has been used on
+    RtHost* rt = nullptr;
+    std::atomic<uint64_t> rt_done{0};
+    unsigned char* rt_dev[64] = {};
 };
 
 std::atomic<int> g_override_kind{-1};   // bg_kernel_info_t.specialised numbering; -1 = default
@@ -49,7 +55,7 @@ struct EnvInit {
         const char* w = getenv("BG_KERNEL_W");
         if (k) {
             g_override_kind = strcmp(k, "general") == 0 ? 0 : strcmp(k, "unit1") == 0 ? 1 :
-                              strcmp(k, "unit2") == 0 ? 2 : strcmp(k, "reg") == 0 ? 3 : -1;
+                              strcmp(k, "unit2") == 0 ? 2 : strcmp(k, "reg") == 0 ? 3 : strcmp(k, "rt") == 0 ? 4 : -1;
         }
         if (w) g_override_w = atoi(w);
     }
@@ -112,6 +118,51 @@ int fill_general(int field, int metric, int n, int d, Launch* L)
     return BG_OK;
 }
 
+const void* rt_ptr(int field, int metric, int d, int s)
+{
+    switch (field) {
+        case BG_FIELD_FP31: return bg_rt_kernel_ptr_fp31(metric, d, s);
+        case BG_FIELD_C128: return bg_rt_kernel_ptr_c128(metric, d, s);
+        case BG_FIELD_FPMONT: return bg_rt_kernel_ptr_mont(metric, d, s);
+    }
+    return nullptr;
+}
+
+// the tiled kernel for a run-time n: one lane per point if a 32-point tile fits shared memory (complex128: two
+// lanes per point first, as in the compiled tables), else two lanes per point, else not available
+int fill_rt(int field, int metric, int n, int d, Launch* L)
+{
+    const int first = field == BG_FIELD_C128 && d % 2 == 0 ? 2 : 1;
+    for (int pass = 0; pass < 2; ++pass) {
+        const int s = pass == 0 ? first : 3 - first;
+        if (d % s != 0) continue;
+        const void* fn = rt_ptr(field, metric, d, s);
+        if (!fn) continue;
+        RtHost* h = new RtHost();
+        if (!bg_rt_make(elem_bytes(field), vec_width(field, d), n, d, s, h) || h->smem > (size_t)kMaxSmemPerBlock) {
+            delete h;
+            continue;
+        }
+        L->func = fn;
+        L->kind = BG_KIND_RT;
+        L->threads = h->threads;
+        L->points_per_block = h->points_per_block;
+        L->smem = (int)h->smem;
+        L->stride = 0;
+        L->rt = h;                                              // (a Launch is filled once; never freed)
+        L->rt_done = 0;
+        return BG_OK;
+    }
+    return BG_ERR_UNSUPPORTED;
+}
+
+// run-time-n shapes: the tiled kernel where it applies, else one thread per point
+int fill_uncompiled(int field, int metric, int n, int d, bool multi_state, Launch* L)
+{
+    if (!multi_state && fill_rt(field, metric, n, d, L) == BG_OK) return BG_OK;
+    return fill_general(field, metric, n, d, L);
+}
+
 void fill_entry(const KernelEntry& e, bool multi, Launch* L)
 {
     L->func = multi ? e.func_multi : e.func;
@@ -146,12 +197,14 @@ int select(int field, int metric, int n, int d, bool multi_state, Launch** out)
         const int key[7] = {ok, ow, field, metric, n, d, (int)multi_state};
         if (memcmp(key, g_over_key, sizeof(key)) != 0) {
             g_over.attr_done = 0;
-            const KernelEntry* e = ok == 0 ? nullptr
-                                           : find_entry(field, metric, n, d, multi_state, ok - 1, ow);
+            const KernelEntry* e = ok == 0 || ok == 4 ? nullptr
+                                                      : find_entry(field, metric, n, d, multi_state, ok - 1, ow);
             int rc = BG_OK;
             if (e) fill_entry(*e, multi_state, &g_over);
-            else if (ok == 0 || !(e = find_entry(field, metric, n, d, multi_state, -1, 0)))
-                rc = fill_general(field, metric, n, d, &g_over);
+            else if (ok == 0) rc = fill_general(field, metric, n, d, &g_over);
+            else if (ok == 4) rc = fill_uncompiled(field, metric, n, d, multi_state, &g_over);
+            else if (!(e = find_entry(field, metric, n, d, multi_state, -1, 0)))
+                rc = fill_uncompiled(field, metric, n, d, multi_state, &g_over);
             else fill_entry(*e, multi_state, &g_over);
             if (rc != BG_OK) { g_over_key[0] = -2; return rc; }
             memcpy(g_over_key, key, sizeof(key));
@@ -168,7 +221,7 @@ int select(int field, int metric, int n, int d, bool multi_state, Launch** out)
         if (s == 0) {
             int rc = BG_OK;
             if (const KernelEntry* e = find_entry(field, metric, n, d, multi_state, -1, 0)) fill_entry(*e, multi_state, L);
-            else rc = fill_general(field, metric, n, d, L);
+            else rc = fill_uncompiled(field, metric, n, d, multi_state, L);
             s = rc == BG_OK ? 1 : 2;
             st.store(s, std::memory_order_release);
         }
@@ -189,6 +242,31 @@ int ensure_attr(Launch* L)
         return BG_ERR_CUDA;
     }
     L->attr_done.fetch_or(bit, std::memory_order_release);
+    return BG_OK;
+}
+
+// the schedule of a run-time-n shape on the current device: allocated and copied at the first call for the shape
+// on that device (a few KB, kept for the life of the process; the one place where the library allocates)
+int ensure_rt_tables(Launch* L, unsigned char** base)
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) { cudaGetLastError(); return BG_ERR_CUDA; }
+    const uint64_t bit = 1ull << dev;
+    if (!(L->rt_done.load(std::memory_order_acquire) & bit)) {
+        std::lock_guard<std::mutex> lock(g_cache_mutex);
+        if (!(L->rt_done.load(std::memory_order_relaxed) & bit)) {
+            void* p = nullptr;
+            if (cudaMalloc(&p, L->rt->blob.size()) != cudaSuccess ||
+                cudaMemcpy(p, L->rt->blob.data(), L->rt->blob.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
+                cudaGetLastError();
+                if (p) cudaFree(p);
+                return BG_ERR_CUDA;
+            }
+            L->rt_dev[dev] = static_cast<unsigned char*>(p);
+            L->rt_done.fetch_or(bit, std::memory_order_release);
+        }
+    }
+    *base = L->rt_dev[dev];
     return BG_OK;
 }
 
@@ -281,6 +359,15 @@ int launch_typed(Launch* L, const bg_problem_t& pb, const typename F::Params& fl
     prm.fld = fld;
     int rc = ensure_attr(L);
     if (rc != BG_OK) return rc;
+    if (L->kind == BG_KIND_RT) {
+        unsigned char* base = nullptr;
+        if ((rc = ensure_rt_tables(L, &base)) != BG_OK) return rc;
+        prm.rt = L->rt->lay;
+        prm.rt_ops = base;
+        prm.rt_quad = reinterpret_cast<const uint32_t*>(base + L->rt->off_quad);
+        prm.rt_beg = reinterpret_cast<const uint16_t*>(base + L->rt->off_beg);
+        prm.rt_ranges = reinterpret_cast<const uint16_t*>(base + L->rt->off_ranges);
+    }
     int64_t blocks = (batch + L->points_per_block - 1) / L->points_per_block;
     if (blocks > 0x7fffffffLL) return BG_ERR_ARG;
     if (L->kind == BG_KIND_REG) {                       // persistent warps: at most the resident blocks of the device
@@ -448,7 +535,7 @@ int bg_amplitudes_primes(int metric, int n, int d, int64_t batch, int n_primes, 
 
 int bg_set_kernel_override(int kind, int warps)
 {
-    g_override_kind = kind < 0 || kind > 3 ? -1 : kind;
+    g_override_kind = kind < 0 || kind > 4 ? -1 : kind;
     g_override_w = warps < 0 ? 0 : warps;
     return BG_OK;
 }
@@ -571,7 +658,7 @@ int bg_kernel_info_problem(const bg_problem_t* problem, bg_kernel_info_t* out)
     Launch* L = nullptr;
     rc = select(problem->field, problem->metric, problem->n, problem->d, problem->states > 1 || problem->orderings, &L);
     if (rc != BG_OK) return rc;
-    out->specialised = L->kind == BG_KIND_GENERAL ? 0 : 1 + L->kind;
+    out->specialised = L->kind == BG_KIND_GENERAL ? 0 : L->kind == BG_KIND_RT ? 4 : 1 + L->kind;
     out->threads_per_block = L->threads;
     out->points_per_block = L->points_per_block;
     out->smem_bytes_per_block = L->smem;

@@ -20,6 +20,16 @@
 
 namespace bg {
 
+// Shared-memory layout of a tile for a run-time n (bg_rt.cuh; the compile-time twin is TileCfg in bg_tile.cuh):
+// vector record rows [0,n) eps, [n, n+r) multi-gluon currents, ps0 + c the doubled prefix sums; scalar tables
+// [index][point]: U per row from 0, V per multi-gluon row from sc_v, 1/P^2 parked in the U slots (sc_w = n),
+// scratch slots of d + 1 entries from sc_scr.  Counts in elements.
+struct RtLayout {
+    int n, m, r;
+    int ps0, vstride;
+    int sc_v, sc_w, sc_scr, nscal, nslots;
+};
+
 // Launch parameters of every recursion kernel.  blockIdx.y = index of the prime of a
 // multi-prime call (0 otherwise): all arrays of prime q start q * (their size) elements in.
 template <class F>
@@ -37,6 +47,12 @@ struct BgParams {
     int n;                // general kernel only
     int stride;           // general kernel only: record stride in elements
     typename F::Params fld;
+    // bg_rt_kernel only (bg_rt.cuh): the tile layout of this n and the schedule, built by the host
+    RtLayout rt;
+    const void* rt_ops;           // FlatOp[]
+    const uint32_t* rt_quad;
+    const uint16_t* rt_beg;       // [W + 1]
+    const uint16_t* rt_ranges;    // [r]: lo | hi << 8 of the proper multi-gluon ranges
 };
 
 template <class F, int D> struct VecWidth { static constexpr int value = 1; };

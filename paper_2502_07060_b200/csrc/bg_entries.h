@@ -9,7 +9,8 @@ enum BgKernelKind {
     BG_KIND_UNIT1 = 0,       // bg_unit_kernel, one lane per point, 32-point tiles
     BG_KIND_UNIT2 = 1,       // bg_unit_kernel, two lanes per point, 16-point tiles
     BG_KIND_REG = 2,         // bg_reg_kernel: currents in registers, no barriers (one state configuration only)
-    BG_KIND_GENERAL = 3      // bg_general_kernel: run-time n, one thread per point (not in the tables)
+    BG_KIND_GENERAL = 3,     // bg_general_kernel: run-time n, one thread per point (not in the tables)
+    BG_KIND_RT = 4           // bg_rt_kernel: the tiled kernel for a run-time n (not in the tables)
 };
 
 struct KernelEntry {
@@ -32,6 +33,12 @@ BG_ENTRY_TABLES(BG_DECLARE_TABLE)
 
 // bg_general_kernel<F, MET, D> for d = 4..16, one translation unit per field (bg_inst_general_*.cu);
 // NULL if (metric, d) is out of range
+// bg_rt_kernel<F, MET, D, kRtWarps, S> for d = 4..16, S = 1 or (even d) 2, one translation unit per field
+// (bg_inst_rt_*.cu); NULL if out of range
+constexpr int kRtWarps = 8;
+const void* bg_rt_kernel_ptr_fp31(int metric, int d, int s);
+const void* bg_rt_kernel_ptr_c128(int metric, int d, int s);
+const void* bg_rt_kernel_ptr_mont(int metric, int d, int s);
 const void* bg_general_kernel_ptr_fp31(int metric, int d);
 const void* bg_general_kernel_ptr_c128(int metric, int d);
 const void* bg_general_kernel_ptr_mont(int metric, int d);

@@ -43,11 +43,16 @@ struct FlatOp {
     uint32_t aux;      // OP_PART: scratch slot (byte offset from the first slot) ; OP_GATHER: mask of slots
 };
 
+// what the operand offsets of an op depend on besides n: element size, tile width and the start of the PS2 rows
+// and of the U / V tables
+struct FlatLayout {
+    int D, EB, TP, PS0, SC_U, SC_V;
+};
+
 template <int N, int W>
-constexpr int flat_count_ops()
+constexpr int flat_count(const LevelProgram<N, W>& p)
 {
     constexpr int M = N - 1;
-    constexpr LevelProgram<N, W> p = LevelProgramOf<N, W>::value;
     int n = 0;
     for (int L = 2; L <= M; ++L)
         for (int w = 0; w < W; ++w) {
@@ -60,11 +65,65 @@ constexpr int flat_count_ops()
         }
     return n;
 }
+template <int N, int W>
+constexpr int flat_count_ops() { return flat_count<N, W>(LevelProgramOf<N, W>::value); }
+constexpr int flat_count_quads(int n) { return n * (n - 1) * (n - 2) * (n - 3) / 24; }
+
+// the ops of the schedule p for the layout y: op[flat_count(p)], quad[flat_count_quads(N)], beg[W + 1].  Evaluated by
+// the compiler for the kernels with a compile-time (n, d), at run time on the host for bg_rt_kernel (bg_api.cu).
+template <int N, int W>
+constexpr void flat_build(const LevelProgram<N, W>& p, const FlatLayout& y, FlatOp* op, uint32_t* quad, uint16_t* beg)
+{
+    constexpr int M = N - 1;
+    static_assert(M * M <= 256 && N + M * (M - 1) / 2 <= 256, "8-bit fields of FlatOp::w");
+    const int D = y.D, EB = y.EB, TP = y.TP, RB = D * EB;
+    int no = 0, nq = 0;
+    for (int w = 0; w < W; ++w) {
+        beg[w] = (uint16_t)no;
+        for (int L = 2; L <= M; ++L) {
+            const int first = no;
+            for (int t = p.beg[L][w]; t < p.beg[L][w + 1]; ++t) {
+                const uint32_t a = p.task[t].a, mask = p.task[t].mask;
+                const int ci = a & 15u, lo = a >> 4 & 15u, hi = a >> 8 & 15u, slot = a >> 12 & 63u;
+                const int own = lv_rowbase<N>(L) + ci;
+                const uint32_t endf = ((a & LT_PART) ? OP_PART : mask ? OP_GATHER | OP_FIN : OP_FIN) |
+                                      (L == M ? OP_TOP : 0u);
+                const uint32_t wfield = (uint32_t)(ci * M + ci + L - 1) | (uint32_t)own << 8 |
+                                        (uint32_t)L << 16 | ((a & LT_PART) ? (uint32_t)(32 * slot) << 20 : 0u);
+                const uint32_t lh = (uint32_t)((y.PS0 + ci) * RB) | (uint32_t)((y.PS0 + ci + L) * RB) << 16;
+                const uint32_t aux = (a & LT_PART) ? (uint32_t)(slot * (D + 1) * TP * EB) : mask;
+                for (int la = lo + 1; la <= hi; ++la) {
+                    FlatOp& o = op[no++];
+                    const int ra = lv_rowbase<N>(la) + ci, rb = lv_rowbase<N>(L - la) + ci + la, c4 = L - la - 1;
+                    o.ab = (uint32_t)(ra * RB) | (uint32_t)(rb * RB) << 16;
+                    o.pso = (uint32_t)((y.PS0 + ci + la) * RB) | (uint32_t)(own * RB) << 16;
+                    o.u = (uint32_t)((y.SC_U + ra) * TP * EB);
+                    o.v = (uint32_t)((rb < N ? y.SC_U + rb : y.SC_V + rb - N) * TP * EB);    // V = U for single gluons
+                    o.w = wfield;
+                    o.lh = lh;
+                    o.aux = aux;
+                    const uint32_t fl = OP_UNIT | (la == lo + 1 ? OP_START : 0u) | (la == hi ? endf : 0u) |
+                                        ((la - lo) % 2 == 1 && la < hi ? OP_PAIR : 0u);
+                    o.qcf = (uint32_t)nq | (uint32_t)c4 << 16 | fl << 24;
+                    for (int lb = 1; lb <= c4; ++lb)
+                        quad[nq++] = (uint32_t)((lv_rowbase<N>(lb) + ci + la) * RB) |
+                                     (uint32_t)((lv_rowbase<N>(L - la - lb) + ci + la + lb) * RB) << 16;
+                }
+            }
+            if (no == first) {                                  // nothing to do at this level but the barrier
+                op[no] = FlatOp{};
+                ++no;
+            }
+            if (L < M) op[no - 1].qcf |= OP_LEND << 24;
+        }
+    }
+    beg[W] = (uint16_t)no;
+}
 
 template <int N, int W>
 struct FlatProgram {
     static constexpr int NOPS = flat_count_ops<N, W>();
-    static constexpr int NQUAD = N * (N - 1) * (N - 2) * (N - 3) / 24;
+    static constexpr int NQUAD = flat_count_quads(N);
     FlatOp op[NOPS];
     uint32_t quad[NQUAD > 0 ? NQUAD : 1];     // row J(k+1..l) | row J(l+1..j) << 16 per 4-gluon split
     uint16_t beg[W + 1];                      // ops of warp w: [beg[w], beg[w+1])
@@ -74,54 +133,34 @@ template <class F, int N, int D, int W, int S>
 constexpr FlatProgram<N, W> make_flat_program()
 {
     typedef TileCfg<F, N, D, W, S, false> C;    // only what does not depend on KW is used below
-    constexpr int M = N - 1, EB = (int)sizeof(typename F::E), TP = C::TP, RB = D * EB;
-    static_assert((long)C::VEC_ROWS * RB < 65536, "row offsets are 16-bit");
-    constexpr LevelProgram<N, W> p = LevelProgramOf<N, W>::value;
+    static_assert((long)C::VEC_ROWS * D * sizeof(typename F::E) < 65536, "row offsets are 16-bit");
     FlatProgram<N, W> f{};
-    int no = 0, nq = 0;
-    for (int w = 0; w < W; ++w) {
-        f.beg[w] = (uint16_t)no;
-        for (int L = 2; L <= M; ++L) {
-            const int first = no;
-            for (int t = p.beg[L][w]; t < p.beg[L][w + 1]; ++t) {
-                const uint32_t a = p.task[t].a, mask = p.task[t].mask;
-                const int ci = a & 15u, lo = a >> 4 & 15u, hi = a >> 8 & 15u, slot = a >> 12 & 63u;
-                const int own = lv_rowbase<N>(L) + ci;
-                const uint32_t endf = ((a & LT_PART) ? OP_PART : mask ? OP_GATHER | OP_FIN : OP_FIN) |
-                                      (L == M ? OP_TOP : 0u);
-                static_assert(M * M <= 256 && N + M * (M - 1) / 2 <= 256, "8-bit fields of FlatOp::w");
-                const uint32_t wfield = (uint32_t)(ci * M + ci + L - 1) | (uint32_t)own << 8 |
-                                        (uint32_t)L << 16 | ((a & LT_PART) ? (uint32_t)(32 * slot) << 20 : 0u);
-                const uint32_t lh = (uint32_t)((C::PS0 + ci) * RB) | (uint32_t)((C::PS0 + ci + L) * RB) << 16;
-                const uint32_t aux = (a & LT_PART) ? (uint32_t)(slot * (D + 1) * TP * EB) : mask;
-                for (int la = lo + 1; la <= hi; ++la) {
-                    FlatOp& o = f.op[no++];
-                    const int ra = lv_rowbase<N>(la) + ci, rb = lv_rowbase<N>(L - la) + ci + la, c4 = L - la - 1;
-                    o.ab = (uint32_t)(ra * RB) | (uint32_t)(rb * RB) << 16;
-                    o.pso = (uint32_t)((C::PS0 + ci + la) * RB) | (uint32_t)(own * RB) << 16;
-                    o.u = (uint32_t)((C::SC_U + ra) * TP * EB);
-                    o.v = (uint32_t)(C::v_index(rb) * TP * EB);
-                    o.w = wfield;
-                    o.lh = lh;
-                    o.aux = aux;
-                    const uint32_t fl = OP_UNIT | (la == lo + 1 ? OP_START : 0u) | (la == hi ? endf : 0u) |
-                                        ((la - lo) % 2 == 1 && la < hi ? OP_PAIR : 0u);
-                    o.qcf = (uint32_t)nq | (uint32_t)c4 << 16 | fl << 24;
-                    for (int lb = 1; lb <= c4; ++lb)
-                        f.quad[nq++] = (uint32_t)((lv_rowbase<N>(lb) + ci + la) * RB) |
-                                       (uint32_t)((lv_rowbase<N>(L - la - lb) + ci + la + lb) * RB) << 16;
-                }
-            }
-            if (no == first) f.op[no++].qcf = 0;               // nothing to do at this level but the barrier
-            if (L < M) f.op[no - 1].qcf |= OP_LEND << 24;
-        }
-    }
-    f.beg[W] = (uint16_t)no;
+    flat_build<N, W>(LevelProgramOf<N, W>::value, FlatLayout{D, (int)sizeof(typename F::E), C::TP, C::PS0, C::SC_U, C::SC_V},
+                     f.op, f.quad, f.beg);
     return f;
 }
 
 template <class F, int N, int D, int W, int S>
 __constant__ FlatProgram<N, W> c_flat_program = make_flat_program<F, N, D, W, S>();
+
+// The finish and the sweep below are written against two small policies, so that the kernels with a compile-time
+// (n, d) and the run-time-n kernel (bg_rt.cuh) share them: the LAYOUT (where the scalar tables start, n) and the
+// PROGRAM (where the ops come from).  For the compile-time kernels both are empty objects whose members fold.
+template <class C>
+struct StaticLay {
+    __device__ __forceinline__ static constexpr int n() { return C::M + 1; }
+    __device__ __forceinline__ static constexpr int sc_u() { return C::SC_U; }
+    __device__ __forceinline__ static constexpr int sc_v() { return C::SC_V; }
+    __device__ __forceinline__ static constexpr int sc_w() { return C::SC_W; }
+    __device__ __forceinline__ static constexpr int sc_scr() { return C::SC_SCR; }
+};
+template <class F, int N, int D, int W, int S>
+struct StaticProg {
+    typedef const FlatOp& Op;
+    __device__ __forceinline__ Op op(int k) const { return c_flat_program<F, N, D, W, S>.op[k]; }
+    __device__ __forceinline__ const uint32_t* quad() const { return c_flat_program<F, N, D, W, S>.quad; }
+    __device__ __forceinline__ int beg(int w) const { return c_flat_program<F, N, D, W, S>.beg[w]; }
+};
 
 // the 4-gluon split (i..k | k+1..l | l+1..j): acc -= 2 (A.C) J(k+1..l); na = -g A
 template <class F, int D, int S>
@@ -263,15 +302,16 @@ __device__ __forceinline__ void unit_pair_body(const F& f, int mu0, const typena
 // Finish the current whose bracket sum is in acc, NEGATED (room for kCapR more products): boundary term of the
 // (P-Q) sum, propagator (the table holds -1/P^2), store, U and V; for the top current the amplitude instead (no
 // propagator).  nx2 = -2 covariant P_{i,j}, nhsum = -sum_k h_k.
-template <class F, int MET, int N, int D, int W, int S, bool KW>
-__device__ __forceinline__ void unit_finish(const F& f, const TileLane<F, N, D, W, S, KW>& t, typename F::E* rec,
+// t: the lane's mu0, half, live, pt.
+template <class F, int MET, int D, int S, class Lay, class Lane>
+__device__ __forceinline__ void unit_finish(const F& f, const Lay& lay, const Lane& t, typename F::E* rec,
                                             typename F::E* sc, const FlatOp& o, bool top,
                                             const typename F::E (&nx2)[D / S], typename F::A (&acc)[D / S],
                                             typename F::E nhsum, typename F::E* out, typename F::E* currents)
 {
-    typedef TileCfg<F, N, D, W, S, KW> C;
     typedef typename F::E E;
-    constexpr int M = N - 1, DL = C::DL, TP = C::TP;
+    constexpr int DL = D / S, TP = 32 / S;
+    const int N = lay.n(), M = N - 1;
     char* rb_ = reinterpret_cast<char*>(rec);
     E l[DL], h[DL];
     ld_vec<F, DL>(reinterpret_cast<const E*>(rb_ + (o.lh & 0xffffu)), l);     // PS2_{i-1}
@@ -292,13 +332,13 @@ __device__ __forceinline__ void unit_finish(const F& f, const TileLane<F, N, D, 
     E v[DL];
     if (!top) {
         const uint32_t own = o.pso >> 16, urow = o.w >> 8 & 0xffu;
-        const E w = sc[(C::SC_W + urow - N) * TP];              // -1/P^2
+        const E w = sc[(lay.sc_w() + urow - N) * TP];           // -1/P^2
 #pragma unroll
         for (int mu = 0; mu < DL; ++mu) v[mu] = f.mul(f.reduce(acc[mu]), w);
         st_vec<F, DL>(reinterpret_cast<E*>(rb_ + own), v);
         const E nc2 = lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, nx2, v)));  // -2 P_{i,j} . J(i..j)
-        sc[(C::SC_U + urow) * TP] = f.canon(f.neg(f.add(nc2, nhsum)));               // U = 2 P.J + sum_k h_k
-        sc[(C::SC_V + urow - N) * TP] = f.sub(nhsum, nc2);                           // V = 2 P.J - sum_k h_k
+        sc[(lay.sc_u() + urow) * TP] = f.canon(f.neg(f.add(nc2, nhsum)));            // U = 2 P.J + sum_k h_k
+        sc[(lay.sc_v() + urow - N) * TP] = f.sub(nhsum, nc2);                        // V = 2 P.J - sum_k h_k
         if (currents && t.live) {
             E* dst = currents + (t.pt * M * M + (long long)(o.w & 0xffu)) * D + t.mu0;
 #pragma unroll
@@ -321,30 +361,28 @@ __device__ __forceinline__ void unit_finish(const F& f, const TileLane<F, N, D, 
 }
 
 // a4-a6 for one state configuration of one tile: the level sweep L = 2..m (Eq.(6)), amplitude, store.
-template <class F, int MET, int N, int D, int W, int S, bool KW>
-__device__ __forceinline__ void unit_sweep_body(const F& f, const TileLane<F, N, D, W, S, KW>& t, const int warp,
-                                                const uint32_t epoch0, typename F::E* out, typename F::E* currents)
+// rec, sc: the lane's record and scalar column; flags: the lane's parked flags, [slot * 32].
+template <class F, int MET, int D, int S, class Lay, class Prog, class Lane>
+__device__ __forceinline__ void unit_sweep_body(const F& f, const Lay& lay, const Prog& prog, const Lane& t,
+                                                const int warp, typename F::E* rec, typename F::E* sc,
+                                                uint32_t* flags, const uint32_t epoch0, typename F::E* out,
+                                                typename F::E* currents)
 {
-    typedef TileCfg<F, N, D, W, S, KW> C;
     typedef typename F::E E;
     typedef typename F::A A;
-    constexpr int DL = C::DL, TP = C::TP;
+    constexpr int DL = D / S, TP = 32 / S, N = 0;              // (N: unused template argument of the unit bodies)
     constexpr bool kPairs = !F::kExact;                         // unit pairs where shared-memory traffic binds
-    const FlatProgram<N, W>& fp = c_flat_program<F, N, D, W, S>;
-    E* rec = t.rec();
-    E* sc = t.sc();
     char* rb_ = reinterpret_cast<char*>(rec);
     char* sb_ = reinterpret_cast<char*>(sc);
-    uint32_t* flags = t.stat + TP + (threadIdx.x & 31);         // this lane's parked flags, [slot * 32]
     E nx2[DL];
     A acc[DL];
     E nhsum = f.ezero();
 #pragma unroll
     for (int mu = 0; mu < DL; ++mu) { nx2[mu] = f.ezero(); acc[mu] = f.zero(); }
-    const int k0 = fp.beg[warp], k1 = fp.beg[warp + 1];
+    const int k0 = prog.beg(warp), k1 = prog.beg(warp + 1);
 #pragma unroll 1
     for (int k = k0; k < k1; ++k) {
-        const FlatOp& o = fp.op[k];
+        typename Prog::Op o = prog.op(k);
         const uint32_t fl = o.qcf >> 24;
         if (fl & OP_START) {
             E l[DL], h[DL];
@@ -357,21 +395,22 @@ __device__ __forceinline__ void unit_sweep_body(const F& f, const TileLane<F, N,
         }
         if constexpr (kPairs) {
             if (fl & OP_PAIR) {
-                unit_pair_body<F, MET, N, D, S>(f, t.mu0, rec, sc, fp.op[k], fp.op[k + 1], fp.quad, nx2, acc, nhsum);
+                typename Prog::Op o2 = prog.op(k + 1);
+                unit_pair_body<F, MET, N, D, S>(f, t.mu0, rec, sc, o, o2, prog.quad(), nx2, acc, nhsum);
                 ++k;                                            // the second unit carries the task's end flags
             } else if (fl & OP_UNIT) {
-                unit_body<F, MET, N, D, S>(f, t.mu0, rec, sc, fp.op[k], fp.quad, nx2, acc, nhsum);
+                unit_body<F, MET, N, D, S>(f, t.mu0, rec, sc, o, prog.quad(), nx2, acc, nhsum);
             }
         } else if (fl & OP_UNIT) {
-            unit_body<F, MET, N, D, S>(f, t.mu0, rec, sc, fp.op[k], fp.quad, nx2, acc, nhsum);
+            unit_body<F, MET, N, D, S>(f, t.mu0, rec, sc, o, prog.quad(), nx2, acc, nhsum);
         }
-        const FlatOp& oe = fp.op[k];                           // the op that carries the task's end flags
+        typename Prog::Op oe = prog.op(k);                     // the op that carries the task's end flags
         const uint32_t fle = oe.qcf >> 24;
         if (fle & OP_PART) {
             // a later part of a current shared between warps: park the partial sums, tell the finisher.
             // (a byte offset from the table, not slot * (D + 1): a run-time multiply here makes ptxas give up the
             // uniform datapath for the whole sweep, +4.5 % at cfg2)
-            E* scr = reinterpret_cast<E*>(sb_ + C::SC_SCR * TP * (int)sizeof(E) + oe.aux);
+            E* scr = reinterpret_cast<E*>(sb_ + lay.sc_scr() * TP * (int)sizeof(E) + oe.aux);
 #pragma unroll
             for (int mu = 0; mu < DL; ++mu) scr[(t.mu0 + mu) * TP] = f.reduce(acc[mu]);
             scr[D * TP] = nhsum;
@@ -396,7 +435,7 @@ __device__ __forceinline__ void unit_sweep_body(const F& f, const TileLane<F, N,
             while (mask) {
                 const int slot = __ffs(mask) - 1;
                 mask &= mask - 1;
-                const E* scr = sc + (C::SC_SCR + slot * (D + 1)) * TP;
+                const E* scr = sc + (lay.sc_scr() + slot * (D + 1)) * TP;
 #pragma unroll
                 for (int mu = 0; mu < DL; ++mu) sum[mu] = f.add(sum[mu], scr[(t.mu0 + mu) * TP]);
                 nhsum = f.add(nhsum, scr[D * TP]);
@@ -405,7 +444,7 @@ __device__ __forceinline__ void unit_sweep_body(const F& f, const TileLane<F, N,
             for (int mu = 0; mu < DL; ++mu) acc[mu] = f.addw(acc[mu], sum[mu]);   // one of the kCapR products of room
         }
         if (fle & OP_FIN)
-            unit_finish<F, MET, N, D, W, S, KW>(f, t, rec, sc, oe, (fle & OP_TOP) != 0, nx2, acc, nhsum, out, currents);
+            unit_finish<F, MET, D, S>(f, lay, t, rec, sc, oe, (fle & OP_TOP) != 0, nx2, acc, nhsum, out, currents);
         if (fle & OP_LEND) __syncthreads();
     }
 }
@@ -483,7 +522,8 @@ __global__ void __launch_bounds__(32 * W, TileCfg<F, N, D, W, S, MULTI>::MIN_BLO
             __syncthreads();
         }
 
-        unit_sweep_body<F, MET, N, D, W, S, KW>(f, t, warp, (uint32_t)(o * states + s) * 16u, gout + s, prm.currents);
+        unit_sweep_body<F, MET, D, S>(f, StaticLay<C>(), StaticProg<F, N, D, W, S>(), t, warp, rec, sc,
+                                      t.stat + TP + lane, (uint32_t)(o * states + s) * 16u, gout + s, prm.currents);
     }
     }
 }

@@ -62,14 +62,17 @@ def test_kernel_info_and_bad_shapes(lib):
     ki = binding.bg_kernel_info(0, 8, 6)
     assert ki["specialised"] >= 1 and ki["points_per_block"] in (16, 32) and ki["threads_per_block"] % 32 == 0
     assert ki["smem_bytes_per_block"] <= 232448
-    assert binding.bg_kernel_info(0, 13, 5)["specialised"] == 0      # outside the compiled grid: general kernel
+    ki = binding.bg_kernel_info(0, 13, 5)                            # outside the compiled grid: run-time-n tiled kernel
+    assert ki["specialised"] == 4 and ki["points_per_block"] == 32 and ki["threads_per_block"] == 256
+    assert binding.bg_kernel_info(0, 16, 16)["points_per_block"] == 16   # two lanes per point: the 32-point tile is too large
+    assert binding.bg_kernel_info_problem(binding.problem(0, 13, 5, states=3))["specialised"] == 0   # general kernel
     assert binding.bg_kernel_info(1, 6, 4)["specialised"] == 3       # cfg1: bg_reg_kernel ...
     pb = binding.problem(1, 6, 4, states=4)
     assert binding.bg_kernel_info_problem(pb)["specialised"] == 2    # ... but not with several state configurations
     for metric in (0, 1):                                            # generic prime, both metrics: compiled cfg2 shape
         pb = binding.problem(binding.FIELD_FPMONT, 8, 6, metric=metric, primes=(2147483629,))
         assert binding.bg_kernel_info_problem(pb)["specialised"] == 1
-    assert binding.bg_kernel_info_problem(binding.problem(0, 7, 7, metric=1))["specialised"] == 0
+    assert binding.bg_kernel_info_problem(binding.problem(0, 7, 7, metric=1))["specialised"] == 4
     big = binding.bg_kernel_info(1, 16, 16)          # largest record: fewer points per block
     assert 1 <= big["threads_per_block"] < 32
     for bad in [(0, 3, 4), (0, 17, 4), (0, 4, 3), (0, 4, 17), (3, 4, 4)]:

@@ -249,8 +249,13 @@ VARIANTS = [("fp31", 8, 6, "unit1", 4), ("fp31", 8, 6, "unit1", 6), ("fp31", 8, 
             ("fp31", 6, 4, "unit1", 2), ("fp31", 8, 4, "unit1", 4), ("fp31", 9, 4, "unit1", 4), ("fp31", 6, 6, "unit1", 2),
             ("fp31", 9, 6, "unit1", 4), ("fp31", 6, 8, "unit1", 2), ("fp31", 8, 8, "unit1", 4), ("fp31", 9, 8, "unit1", 4),
             ("fp31", 6, 10, "unit1", 2), ("fp31", 9, 10, "unit1", 4), ("fp31", 5, 4, "unit1", 1), ("fp31", 7, 4, "unit1", 4),
-            ("fp31", 10, 4, "unit1", 8), ("fp31", 4, 8, "unit1", 1), ("fp31", 5, 8, "unit1", 1), ("fp31", 7, 8, "unit1", 4)]
-KIND_ID = {"general": 0, "unit1": 1, "unit2": 2, "reg": 3}
+            ("fp31", 10, 4, "unit1", 8), ("fp31", 4, 8, "unit1", 1), ("fp31", 5, 8, "unit1", 1), ("fp31", 7, 8, "unit1", 4),
+            # the tiled kernel for a run-time n (bg_rt_kernel): shapes with and without a compiled instance, one
+            # and two lanes per point, odd d
+            ("fp31", 8, 6, "rt", 8), ("fp31", 4, 4, "rt", 8), ("fp31", 13, 5, "rt", 8), ("fp31", 16, 4, "rt", 8),
+            ("fp31", 5, 16, "rt", 8), ("fp31", 11, 9, "rt", 8), ("fp31", 16, 16, "rt", 8),
+            ("c128", 6, 4, "rt", 8), ("c128", 12, 6, "rt", 8), ("c128", 7, 5, "rt", 8), ("c128", 13, 4, "rt", 8)]
+KIND_ID = {"general": 0, "unit1": 1, "unit2": 2, "reg": 3, "rt": 4}
 
 
 @pytest.mark.parametrize("field,n,d,kernel,w", VARIANTS, ids=lambda v: str(v))
@@ -332,7 +337,8 @@ EXTREME_CASES = [(8, 6, "unit1", 4), (8, 6, "unit1", 6), (8, 6, "unit1", 2), (8,
                  (12, 6, "unit1", 8), (12, 6, "unit1", 16), (12, 6, "general", 0),
                  (10, 8, "unit1", 8), (10, 8, "unit1", 4), (10, 8, "general", 0),
                  (4, 4, "unit1", 1), (4, 4, "general", 0), (9, 10, "unit1", 4), (7, 5, "unit1", 4),
-                 (5, 16, "general", 0), (16, 4, "general", 0), (16, 16, "general", 0)]
+                 (5, 16, "general", 0), (16, 4, "general", 0), (16, 16, "general", 0),
+                 (8, 6, "rt", 8), (13, 5, "rt", 8), (16, 4, "rt", 8), (5, 16, "rt", 8), (16, 16, "rt", 8)]
 
 
 @pytest.mark.parametrize("n,d,kernel,w", EXTREME_CASES, ids=lambda v: str(v))
@@ -349,3 +355,20 @@ def test_fp_extreme_residues(bgl, oracle_mod, select_kernel, n, d, kernel, w):
         assert np.array_equal(bgl.to_numpy(out), ref), kind
         assert np.array_equal(bgl.to_numpy(cur)[:, iu[0], iu[1]], rcur[:, iu[0], iu[1]]), kind
         assert np.array_equal(st.cpu().numpy().astype(np.uint32), rst), kind
+
+
+def test_uncompiled_shapes_run_the_tiled_kernel_and_match_the_compiled_one(bgl, oracle_mod, select_kernel):
+    """shapes without a compiled instance default to bg_rt_kernel (one state configuration, one ordering); on a
+    compiled shape it gives the same residues as the compiled kernel, status words included"""
+    assert bgl.bg_kernel_info(bgl.FIELD_FP31, 13, 5)["specialised"] == 4
+    assert bgl.bg_kernel_info(bgl.FIELD_FP31, 8, 6)["specialised"] == 1
+    mom, pol, _ = inputs.make_fp_inputs(10, 8, 1000, seed=5)
+    mom[7, 1] = mom[7, 0]                                    # a vanishing invariant: inv(0) := 0, status bit 0
+    dm, dp = bgl.to_device(mom), bgl.to_device(pol)
+    import torch
+    st0 = torch.zeros(1000, dtype=torch.int32, device="cuda")
+    a = bgl.to_numpy(bgl.amplitudes(dm, dp, status=st0))
+    select_kernel("rt", 0)
+    st1 = torch.zeros(1000, dtype=torch.int32, device="cuda")
+    b = bgl.to_numpy(bgl.amplitudes(dm, dp, status=st1))
+    assert np.array_equal(a, b) and torch.equal(st0, st1) and int(st0[7]) == 1
