@@ -224,7 +224,8 @@ def _state_sum_definition(amps, prime=None):
     return (prod.sum(axis=1) % prime).astype(np.uint32)
 
 
-@pytest.mark.parametrize("trees,S,batch", [(1, 1, 70), (2, 16, 1000), (3, 4, 333), (8, 5, 65)])
+@pytest.mark.parametrize("trees,S,batch", [(1, 1, 70), (2, 16, 1000), (3, 4, 333), (8, 5, 65), (2, 8, 1001), (3, 32, 257),
+                                           (2, 64, 100), (2, 128, 77), (2, 12, 99), (4, 256, 9)])
 def test_state_sum_fp(bgl, trees, S, batch):
     import torch
     rng = np.random.default_rng(trees * 100 + S)
