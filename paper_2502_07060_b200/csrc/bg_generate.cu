@@ -14,8 +14,8 @@
 //     vanishing M00 of k_i or r_i) are redrawn with attempt + 1.
 //
 // Over F_p the output is bit-identical to inputs.py (exact arithmetic); over complex128 it agrees to
-// rounding (numpy sums and divides in its own order).  All inversions of a point go through
-// Montgomery's trick in three rounds (light-cone 1/(2p+), alpha, polarisation coefficients).
+// rounding (numpy sums and divides in its own order).  The 2n-1 light-cone 1/(2p+) go through Montgomery's
+// trick; alpha and the polarisation coefficient of every leg cost one field inversion each.
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -88,6 +88,11 @@ struct Draws {
     }
 };
 
+// (not inlined: four call sites of a 38-multiplication chain took the kernel to 59 KB of code, past the instruction
+// cache: `no_instruction` 23 % of the stall samples)
+template <class F>
+__device__ __noinline__ typename F::E inv_call(const F& f, typename F::E a) { return f.inv(a); }
+
 template <class F>
 __device__ __forceinline__ typename F::E mdot(const F& f, int metric, int d, const typename F::E* x,
                                               const typename F::E* y)
@@ -134,7 +139,7 @@ __global__ void __launch_bounds__(128) generate_kernel(const GenParams<F> prm)
     const bool live = pt < prm.batch;
 
     if (live) {
-        E km[MAXND], ep[MAXND], rr[MAXND], scr[4 * 16 + 2];    // momenta; v_i then eps_i; r_i; inverses and dots
+        E km[MAXND], scr[4 * 16];                              // momenta; the light-cone inverses and 2 p+
         const uint64_t index = (uint64_t)(prm.start + pt);
         const int eq = (n - 2) * (d - 1);                      // first stream element of q
         const int ev = (n - 1) * (d - 1);                      // first stream element of the (v_i, r_i) block
@@ -151,19 +156,20 @@ __global__ void __launch_bounds__(128) generate_kernel(const GenParams<F> prm)
                 return j < n - 2 ? j * (d - 1) : j == n - 2 ? eq : ev + (j - (n - 1)) * (2 * d - 1) + d;
             };
             if constexpr (F::kExact) {
+                E* xp = scr + 32;                              // 2 p+ of every light-cone vector: drawn once
                 E c = f.one();
                 for (int j = 0; j < 2 * n - 1; ++j) {
                     invA[j] = c;
-                    c = f.mul(c, f.dbl(dr.nonzero(plus_elem(j))));
+                    xp[j] = f.dbl(dr.nonzero(plus_elem(j)));
+                    c = f.mul(c, xp[j]);
                 }
-                E u = f.inv(c);
+                E u = inv_call<F>(f, c);
                 for (int j = 2 * n - 2; j >= 0; --j) {
-                    const E x = f.dbl(dr.nonzero(plus_elem(j)));
                     invA[j] = f.mul(u, invA[j]);
-                    u = f.mul(u, x);
+                    u = f.mul(u, xp[j]);
                 }
             } else {
-                for (int j = 0; j < 2 * n - 1; ++j) invA[j] = f.inv(f.dbl(dr.nonzero(plus_elem(j))));
+                for (int j = 0; j < 2 * n - 1; ++j) invA[j] = inv_call<F>(f, f.dbl(dr.nonzero(plus_elem(j))));
             }
             // ---- momenta ---------------------------------------------------------------------------------
             E ksum[bg::kMaxD], q[bg::kMaxD];
@@ -176,67 +182,48 @@ __global__ void __launch_bounds__(128) generate_kernel(const GenParams<F> prm)
             for (int mu = 0; mu < d; ++mu) ksum[mu] = f.canon(f.neg(ksum[mu]));           // K
             const E K2 = mdot<F>(f, metric, d, ksum, ksum), Kq = mdot<F>(f, metric, d, ksum, q);
             if (F::kExact && f.is_zero(f.canon(Kq))) ok = false;
-            const E alpha = f.mul(K2, f.inv(f.dbl(Kq)));                                   // round B
+            const E alpha = f.mul(K2, inv_call<F>(f, f.dbl(Kq)));                                   // round B
             for (int mu = 0; mu < d; ++mu) {
                 const E a = f.mul(alpha, q[mu]);
                 km[(n - 2) * d + mu] = a;
                 km[(n - 1) * d + mu] = f.sub(ksum[mu], a);
             }
-            // ---- polarisations: v_i, r_i, then eps_i -----------------------------------------------------
-            E* den = scr + 2 * n;                              // [n]   r_i.p_i  (or the spinor denominators)
-            E* num = scr + 3 * n;                              // [n]   v_i.p_i
+            // ---- polarisations, leg by leg: v_i, r_i, eps_i = v_i - (v_i.p_i)/(r_i.p_i) r_i (or the helicity state on
+            //      (k_i, r_i)), stored at once (a redraw overwrites them).  One field inversion per leg instead of
+            //      Montgomery's trick over the legs: that needed every v_i and r_i kept until the common inverse was
+            //      known -- 2 n d more words of thread-local memory, which spilled through L2 into HBM (3.2 GB of DRAM
+            //      traffic per 2^20 cfg2 points against 0.8 GB of output, `long_scoreboard` 73 % of the stall samples).
+            E* gp = prm.pol + pt * nd;
+            E* gr = prm.ref ? prm.ref + pt * nd : nullptr;
             for (int i = 0; i < n; ++i) {
                 const int e0 = ev + i * (2 * d - 1);
-                for (int mu = 0; mu < d; ++mu) ep[i * d + mu] = dr.any(e0 + mu);
-                massless<F>(f, dr, metric, d, e0 + d, invA[n - 1 + i], rr + i * d);
-                const E rp = mdot<F>(f, metric, d, rr + i * d, km + i * d);
-                if (F::kExact && f.is_zero(f.canon(rp))) ok = false;
-                den[i] = rp;
-                num[i] = mdot<F>(f, metric, d, ep + i * d, km + i * d);
-            }
-            if (prm.use_hel) {
-                // spinor-helicity states on (k_i, r_i), unnormalised spinors (bg_states.cuh):
-                //   eps_- = vec(lam_k lamt'_r^T) M00(k) / [r k]',  eps_+ = 2 vec(lam_r lamt'_k^T) / (M00(k) <r k>)
-                for (int i = 0; i < n; ++i) {
-                    E lk[2], ltk[2], lr[2], ltr[2];
-                    bg::spinors_unnormalised<F>(f, prm.sc, km + i * d, lk, ltk);
-                    bg::spinors_unnormalised<F>(f, prm.sc, rr + i * d, lr, ltr);
-                    if (F::kExact && (f.is_zero(f.canon(lk[0])) || f.is_zero(f.canon(lr[0])))) ok = false;
-                    den[i] = prm.hel[i] < 0 ? f.sub(f.mul(ltr[0], ltk[1]), f.mul(ltr[1], ltk[0]))
-                                            : f.mul(lk[0], f.sub(f.mul(lr[0], lk[1]), f.mul(lr[1], lk[0])));
-                }
-            }
-            // round C: 1/den_i for all legs at once (zero-safe)
-            if constexpr (F::kExact) {
-                E* pre = scr;                                  // invA is no longer needed
-                E c = f.one();
-                for (int i = 0; i < n; ++i) {
-                    pre[i] = c;
-                    const bool z = f.is_zero(f.canon(den[i]));
-                    c = f.mul(c, z ? f.one() : den[i]);
-                }
-                E u = f.inv(c);
-                for (int i = n - 1; i >= 0; --i) {
-                    const bool z = f.is_zero(f.canon(den[i]));
-                    const E x = den[i];
-                    den[i] = z ? f.ezero() : f.mul(u, pre[i]);
-                    u = f.mul(u, z ? f.one() : x);
-                }
-            } else {
-                for (int i = 0; i < n; ++i) den[i] = f.inv(den[i]);
-            }
-            for (int i = 0; i < n; ++i) {
-                if (prm.use_hel) {
-                    E lk[2], ltk[2], lr[2], ltr[2], v4[4];
-                    bg::spinors_unnormalised<F>(f, prm.sc, km + i * d, lk, ltk);
-                    bg::spinors_unnormalised<F>(f, prm.sc, rr + i * d, lr, ltr);
-                    if (prm.hel[i] < 0) bg::bispinor_vec<F>(f, prm.sc, lk, ltr, f.mul(lk[0], den[i]), v4);
-                    else bg::bispinor_vec<F>(f, prm.sc, lr, ltk, f.dbl(den[i]), v4);
-                    for (int mu = 0; mu < 4; ++mu) ep[i * d + mu] = v4[mu];
+                E v[bg::kMaxD], r[bg::kMaxD];
+                for (int mu = 0; mu < d; ++mu) v[mu] = dr.any(e0 + mu);
+                massless<F>(f, dr, metric, d, e0 + d, invA[n - 1 + i], r);
+                const E* k = km + i * d;
+                if (!prm.use_hel) {
+                    const E rp = mdot<F>(f, metric, d, r, k);
+                    if (F::kExact && f.is_zero(f.canon(rp))) ok = false;
+                    const E coef = f.mul(mdot<F>(f, metric, d, v, k), inv_call<F>(f, f.canon(rp)));      // inv(0) = 0
+                    for (int mu = 0; mu < d; ++mu) v[mu] = f.sub(v[mu], f.mul(coef, r[mu]));
                 } else {
-                    const E coef = f.mul(num[i], den[i]);
-                    for (int mu = 0; mu < d; ++mu)
-                        ep[i * d + mu] = f.sub(ep[i * d + mu], f.mul(coef, rr[i * d + mu]));
+                    // spinor-helicity states on (k_i, r_i), unnormalised spinors (bg_states.cuh):
+                    //   eps_- = vec(lam_k lamt'_r^T) M00(k) / [r k]',  eps_+ = 2 vec(lam_r lamt'_k^T) / (M00(k) <r k>)
+                    E lk[2], ltk[2], lr[2], ltr[2], v4[4];
+                    bg::spinors_unnormalised<F>(f, prm.sc, k, lk, ltk);
+                    bg::spinors_unnormalised<F>(f, prm.sc, r, lr, ltr);
+                    if (F::kExact && (f.is_zero(f.canon(lk[0])) || f.is_zero(f.canon(lr[0])))) ok = false;
+                    const E den = prm.hel[i] < 0 ? f.sub(f.mul(ltr[0], ltk[1]), f.mul(ltr[1], ltk[0]))
+                                                 : f.mul(lk[0], f.sub(f.mul(lr[0], lk[1]), f.mul(lr[1], lk[0])));
+                    if (F::kExact && f.is_zero(f.canon(den))) ok = false;
+                    const E dinv = inv_call<F>(f, f.canon(den));
+                    if (prm.hel[i] < 0) bg::bispinor_vec<F>(f, prm.sc, lk, ltr, f.mul(lk[0], dinv), v4);
+                    else bg::bispinor_vec<F>(f, prm.sc, lr, ltk, f.dbl(dinv), v4);
+                    for (int mu = 0; mu < 4; ++mu) v[mu] = v4[mu];
+                }
+                for (int mu = 0; mu < d; ++mu) {
+                    gp[i * d + mu] = f.to_output(v[mu]);
+                    if (gr) gr[i * d + mu] = f.to_output(r[mu]);
                 }
             }
             // ---- F_p: reject points with a vanishing proper invariant P_{i,j}^2 ------------------------------
@@ -257,15 +244,7 @@ __global__ void __launch_bounds__(128) generate_kernel(const GenParams<F> prm)
         if (attempt && prm.redraws) atomicAdd(prm.redraws, (unsigned long long)attempt);
         // every thread stores its own point (n d contiguous elements per array; L2 merges the sectors)
         E* gm = prm.mom + pt * nd;
-        E* gp = prm.pol + pt * nd;
-        for (int w = 0; w < nd; ++w) {
-            gm[w] = f.to_output(km[w]);
-            gp[w] = f.to_output(ep[w]);
-        }
-        if (prm.ref) {
-            E* gr = prm.ref + pt * nd;
-            for (int w = 0; w < nd; ++w) gr[w] = f.to_output(rr[w]);
-        }
+        for (int w = 0; w < nd; ++w) gm[w] = f.to_output(km[w]);
     }
 }
 
