@@ -31,7 +31,7 @@ def _vectors(field, d, count, seed, metric, prime):
 
 
 # ---- bg_states ----------------------------------------------------------------------------------------
-@pytest.mark.parametrize("d", range(4, 11))
+@pytest.mark.parametrize("d", list(range(4, 11)) + [13, 16])
 @pytest.mark.parametrize("metric,prime", [(1, 0), (1, PRIMES[0]), (1, PRIMES[2]), (0, P_1MOD4), (1, P_1MOD4)])
 def test_states_fp_bit_exact(bgl, d, metric, prime):
     import torch
