@@ -57,7 +57,7 @@ def test_montgomery_with_the_mersenne_prime_equals_fp31(bgl, n, d):
     assert np.array_equal(a, b)
 
 
-@pytest.mark.parametrize("n,d", [(8, 6), (6, 5)])
+@pytest.mark.parametrize("n,d", [(8, 6), (6, 5), (11, 7), (13, 4)])      # the last two: no compiled instance (bg_rt_kernel)
 def test_several_primes_in_one_launch(bgl, oracle_mod, n, d):
     batch = 77
     primes = (PRIMES[0], PRIMES[2], P31, PRIMES[1])
