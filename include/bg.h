@@ -38,10 +38,7 @@
  *   limits    4 <= n <= 16, 4 <= d <= 16 (the paper validates d = 4..10).
  *   memory    the caller owns every buffer; DEVICE pointers unless the name says host.
  *             Device pointers must be 16-byte aligned; out must not alias the inputs.
- *             The library keeps no per-call state and allocates no device memory, with one exception:
- *             the first call for a shape (n, d) that has no compiled instance copies the work
- *             schedule of that shape to the device it runs on (a few KB per shape and device, built
- *             on the host, kept for the life of the process; that first call is synchronous).
+ *             The library allocates no device memory and keeps no per-call state.
  *   stream    launches are asynchronous on `stream`; nothing synchronises.
  *   errors    return value: BG_OK or a negative bg_status_t; nothing is thrown, nothing
  *             aborts.  Arguments are checked on the host before any launch.  batch == 0 is

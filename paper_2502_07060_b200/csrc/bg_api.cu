@@ -38,11 +38,9 @@ struct Launch {
     int smem = 0;
     int stride = 0;                    // general kernel: record stride in elements
     std::atomic<uint64_t> attr_done{0};   // bit i: cudaFuncSetAttribute done on device i
-    // bg_rt_kernel: layout and schedule built by the host (kept for the life of the process), and the copy of
-    // the tables on every device the shape has been used on
+    // bg_rt_kernel: layout and schedule built by the host (kept for the life of the process); every launch
+    // carries them in its parameter block
     RtHost* rt = nullptr;
-    std::atomic<uint64_t> rt_done{0};
-    unsigned char* rt_dev[64] = {};
 };
 
 std::atomic<int> g_override_kind{-1};   // bg_kernel_info_t.specialised numbering; -1 = default
@@ -150,7 +148,6 @@ int fill_rt(int field, int metric, int n, int d, Launch* L)
         L->smem = (int)h->smem;
         L->stride = 0;
         L->rt = h;                                              // (a Launch is filled once; never freed)
-        L->rt_done = 0;
         return BG_OK;
     }
     return BG_ERR_UNSUPPORTED;
@@ -245,31 +242,6 @@ int ensure_attr(Launch* L)
     return BG_OK;
 }
 
-// the schedule of a run-time-n shape on the current device: allocated and copied at the first call for the shape
-// on that device (a few KB, kept for the life of the process; the one place where the library allocates)
-int ensure_rt_tables(Launch* L, unsigned char** base)
-{
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) { cudaGetLastError(); return BG_ERR_CUDA; }
-    const uint64_t bit = 1ull << dev;
-    if (!(L->rt_done.load(std::memory_order_acquire) & bit)) {
-        std::lock_guard<std::mutex> lock(g_cache_mutex);
-        if (!(L->rt_done.load(std::memory_order_relaxed) & bit)) {
-            void* p = nullptr;
-            if (cudaMalloc(&p, L->rt->blob.size()) != cudaSuccess ||
-                cudaMemcpy(p, L->rt->blob.data(), L->rt->blob.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
-                cudaGetLastError();
-                if (p) cudaFree(p);
-                return BG_ERR_CUDA;
-            }
-            L->rt_dev[dev] = static_cast<unsigned char*>(p);
-            L->rt_done.fetch_or(bit, std::memory_order_release);
-        }
-    }
-    *base = L->rt_dev[dev];
-    return BG_OK;
-}
-
 }  // namespace
 
 // ---- Montgomery constants of a prime (also used by bg_state_sum.cu) ----------------------------------
@@ -359,15 +331,7 @@ int launch_typed(Launch* L, const bg_problem_t& pb, const typename F::Params& fl
     prm.fld = fld;
     int rc = ensure_attr(L);
     if (rc != BG_OK) return rc;
-    if (L->kind == BG_KIND_RT) {
-        unsigned char* base = nullptr;
-        if ((rc = ensure_rt_tables(L, &base)) != BG_OK) return rc;
-        prm.rt = L->rt->lay;
-        prm.rt_ops = base;
-        prm.rt_quad = reinterpret_cast<const uint32_t*>(base + L->rt->off_quad);
-        prm.rt_beg = reinterpret_cast<const uint16_t*>(base + L->rt->off_beg);
-        prm.rt_ranges = reinterpret_cast<const uint16_t*>(base + L->rt->off_ranges);
-    }
+    if (L->kind == BG_KIND_RT) prm.rt = L->rt->lay;
     int64_t blocks = (batch + L->points_per_block - 1) / L->points_per_block;
     if (blocks > 0x7fffffffLL) return BG_ERR_ARG;
     if (L->kind == BG_KIND_REG) {                       // persistent warps: at most the resident blocks of the device
@@ -375,8 +339,16 @@ int launch_typed(Launch* L, const bg_problem_t& pb, const typename F::Params& fl
         if (resident > 0 && blocks > resident) blocks = resident;
     }
     const unsigned gy = pb.field == BG_FIELD_FPMONT ? (unsigned)pb.n_primes : 1u;
-    void* args[] = {&prm};
-    if (cudaLaunchKernel(L->func, dim3((unsigned)blocks, gy), dim3(L->threads), args, L->smem, stream) != cudaSuccess) {
+    bg::RtParams<F>* rp = nullptr;
+    if (L->kind == BG_KIND_RT) {                        // the schedule travels in the parameter block (29 KB)
+        rp = new bg::RtParams<F>;
+        rp->base = prm;
+        rp->tab = L->rt->tab;
+    }
+    void* args[] = {rp ? static_cast<void*>(rp) : static_cast<void*>(&prm)};
+    const cudaError_t err = cudaLaunchKernel(L->func, dim3((unsigned)blocks, gy), dim3(L->threads), args, L->smem, stream);
+    delete rp;                                          // cudaLaunchKernel has copied the parameters
+    if (err != cudaSuccess) {
         cudaGetLastError();
         return BG_ERR_CUDA;
     }

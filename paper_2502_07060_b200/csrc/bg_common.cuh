@@ -47,13 +47,37 @@ struct BgParams {
     int n;                // general kernel only
     int stride;           // general kernel only: record stride in elements
     typename F::Params fld;
-    // bg_rt_kernel only (bg_rt.cuh): the tile layout of this n and the schedule, built by the host
-    RtLayout rt;
-    const void* rt_ops;           // FlatOp[]
-    const uint32_t* rt_quad;
-    const uint16_t* rt_beg;       // [W + 1]
-    const uint16_t* rt_ranges;    // [r]: lo | hi << 8 of the proper multi-gluon ranges
+    RtLayout rt;          // bg_rt_kernel only (bg_rt.cuh): the tile layout of this n
 };
+
+// One op of the flat per-warp program of the tiled kernels (bg_unit.cuh: flat_build, unit_sweep_body).
+struct FlatOp {
+    uint32_t ab;       // row A | row B << 16      (byte offsets in the lane's vector record)
+    uint32_t pso;      // row PS2_k | own row << 16
+    uint32_t u, v;     // U_A, V_B                 (byte offsets from the lane's scalar base)
+    uint32_t w;        // ci * m + j - 1 (position in the caller's `currents` array) | own row << 8 | level << 16
+                       // | OP_PART: first parked flag of the slot (word index) << 20
+    uint32_t lh;       // rows PS2_{i-1} | PS2_j << 16
+    uint32_t qcf;      // first entry of the op's 4-gluon splits in quad[] | c4 << 16 | flags << 24
+    uint32_t aux;      // OP_PART: scratch slot (byte offset from the first slot) ; OP_GATHER: mask of slots
+};
+
+// bg_rt_kernel: the schedule of a run-time n travels with the launch as a kernel PARAMETER (constant bank: the ops
+// are read with uniform loads like the __constant__ tables of the compiled kernels; nothing is allocated or copied
+// to the device).  Sized for n = 16 with kRtWarps = 8 warps; 29 KB of the 32 KB a kernel may take.
+constexpr int kRtMaxOps = 680, kRtMaxQuad = 1820, kRtMaxRanges = 104;
+struct RtTables {
+    FlatOp ops[kRtMaxOps];
+    uint32_t quad[kRtMaxQuad];    // row J(k+1..l) | row J(l+1..j) << 16 per 4-gluon split
+    uint16_t beg[16];             // ops of warp w: [beg[w], beg[w+1])
+    uint16_t ranges[kRtMaxRanges];   // lo | hi << 8 of the proper multi-gluon ranges
+};
+template <class F>
+struct RtParams {
+    BgParams<F> base;
+    RtTables tab;
+};
+static_assert(sizeof(RtTables) + 512 <= 32764, "kernel parameters are limited to 32764 bytes");
 
 template <class F, int D> struct VecWidth { static constexpr int value = 1; };
 template <int D> struct VecWidth<Fp31, D> { static constexpr int value = (D % 4 == 0) ? 4 : (D % 2 == 0) ? 2 : 1; };

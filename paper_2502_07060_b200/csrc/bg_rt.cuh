@@ -4,8 +4,9 @@
 // Same tile (32 / S points, W warps, per-point records with an odd stride, scalar tables [index][point]), same
 // schedule (bg_schedule.cuh), same flat op program, same unit bodies, finish and sweep as bg_unit_kernel
 // (bg_unit.cuh: unit_split3 / unit_body / unit_pair_body / unit_finish / unit_sweep_body, shared through the layout
-// and program policies) -- but the layout is a kernel argument and the ops are built by the host at the first call
-// for a shape and read from global memory (bg_api.cu: rt_tables).  Only the per-tile setup (rows a0-a3) is
+// and program policies) -- but the layout and the ops are kernel ARGUMENTS: the host builds the schedule at the first
+// call for a shape (bg_rt_host.cu) and every launch carries it in its parameter block (RtParams, bg_common.cuh: the
+// constant bank, read with uniform loads like the compiled kernels' tables).  Only the per-tile setup (rows a0-a3) is
 // restated here with run-time row counts.  One state configuration and one colour ordering per point; requests
 // with more of either, and shapes whose 16-point tile does not fit shared memory, run bg_general_kernel.
 //
@@ -25,22 +26,12 @@ struct RtLay {
     __device__ __forceinline__ int sc_scr() const { return l.sc_scr; }
 };
 
-struct RtProg {
-    typedef FlatOp Op;                                          // by value: two 16-byte loads through the read-only path
-    const FlatOp* ops;
-    const uint32_t* q;
-    const uint16_t* b;
-    __device__ __forceinline__ Op op(int k) const
-    {
-        const uint4* p = reinterpret_cast<const uint4*>(ops + k);
-        const uint4 x = __ldg(p), y = __ldg(p + 1);
-        FlatOp o;
-        o.ab = x.x; o.pso = x.y; o.u = x.z; o.v = x.w;
-        o.w = y.x; o.lh = y.y; o.qcf = y.z; o.aux = y.w;
-        return o;
-    }
-    __device__ __forceinline__ const uint32_t* quad() const { return q; }
-    __device__ __forceinline__ int beg(int w) const { return __ldg(b + w); }
+struct RtProg {                                                 // the tables are a kernel parameter: constant bank
+    typedef const FlatOp& Op;
+    const RtTables& tab;
+    __device__ __forceinline__ Op op(int k) const { return tab.ops[k]; }
+    __device__ __forceinline__ const uint32_t* quad() const { return tab.quad; }
+    __device__ __forceinline__ int beg(int w) const { return tab.beg[w]; }
 };
 
 struct RtLane {
@@ -67,8 +58,9 @@ __device__ __forceinline__ void rt_stage(const F& f, typename F::E* vec, int vst
 }
 
 template <class F, int MET, int D, int W, int S>
-__global__ void __launch_bounds__(32 * W) bg_rt_kernel(const BgParams<F> prm)
+__global__ void __launch_bounds__(32 * W) bg_rt_kernel(const __grid_constant__ RtParams<F> P)
 {
+    const BgParams<F>& prm = P.base;
     typedef typename F::E E;
     typedef typename F::A A;
     constexpr int TP = 32 / S, DL = D / S;
@@ -146,7 +138,7 @@ __global__ void __launch_bounds__(32 * W) bg_rt_kernel(const BgParams<F> prm)
         uint32_t status = 0;
 #pragma unroll 1
         for (int r = vw; r < L.r; r += VW) {
-            const uint32_t rg = __ldg(prm.rt_ranges + r);
+            const uint32_t rg = P.tab.ranges[r];
             E lo[D], hi[D], x[D], nx[D];
             ld_vec<F, D>(recf + (PS0 + (rg & 255u)) * D, lo);
             ld_vec<F, D>(recf + (PS0 + (rg >> 8)) * D, hi);
@@ -192,10 +184,7 @@ __global__ void __launch_bounds__(32 * W) bg_rt_kernel(const BgParams<F> prm)
     // ---- a4-a6: the level sweep (bg_unit.cuh) ----
     RtLay lay;
     lay.l = L;
-    RtProg prog;
-    prog.ops = static_cast<const FlatOp*>(prm.rt_ops);
-    prog.q = prm.rt_quad;
-    prog.b = prm.rt_beg;
+    const RtProg prog{P.tab};
     unit_sweep_body<F, MET, D, S>(f, lay, prog, t, warp, rec, sc, stat + TP + lane, 0u, prm.out + pbase + t.pt,
                                   prm.currents);
 }

@@ -11,7 +11,7 @@
 namespace {
 
 template <int N>
-void make_for(int eb, int u, int d, int s, RtHost* out)
+bool make_for(int eb, int u, int d, int s, RtHost* out)
 {
     constexpr int W = kRtWarps, M = N - 1, R = M * (M - 1) / 2 - 1;
     const bg::LevelProgram<N, W> p = bg::make_level_program<N, W>();
@@ -31,24 +31,15 @@ void make_for(int eb, int u, int d, int s, RtHost* out)
     out->threads = 32 * W;
     out->points_per_block = tp;
     out->smem = (size_t)tp * (L.vstride + L.nscal) * eb + (size_t)(tp + 32 * L.nslots) * sizeof(uint32_t);
-    const int nops = bg::flat_count<N, W>(p), nquad = bg::flat_count_quads(N);
-    std::vector<bg::FlatOp> ops(nops);
-    std::vector<uint32_t> quad(nquad > 0 ? nquad : 1);
-    uint16_t beg[W + 1];
-    bg::flat_build<N, W>(p, bg::FlatLayout{d, eb, tp, L.ps0, 0, L.sc_v}, ops.data(), quad.data(), beg);
-    std::vector<uint16_t> ranges(R > 0 ? R : 1);
+    static_assert(W + 1 <= 16, "RtTables::beg");
+    memset(&out->tab, 0, sizeof(out->tab));
+    if (bg::flat_count<N, W>(p) > bg::kRtMaxOps || bg::flat_count_quads(N) > bg::kRtMaxQuad || R > bg::kRtMaxRanges)
+        return false;
+    bg::flat_build<N, W>(p, bg::FlatLayout{d, eb, tp, L.ps0, 0, L.sc_v}, out->tab.ops, out->tab.quad, out->tab.beg);
     int r = 0;
     for (int len = 2; len <= N - 2; ++len)
-        for (int i = 0; i + len <= N - 1; ++i) ranges[r++] = (uint16_t)(i | (i + len) << 8);
-    auto align16 = [](size_t x) { return (x + 15) & ~(size_t)15; };
-    out->off_quad = align16(ops.size() * sizeof(bg::FlatOp));
-    out->off_beg = align16(out->off_quad + quad.size() * sizeof(uint32_t));
-    out->off_ranges = align16(out->off_beg + sizeof(beg));
-    out->blob.assign(align16(out->off_ranges + ranges.size() * sizeof(uint16_t)), 0);
-    memcpy(out->blob.data(), ops.data(), ops.size() * sizeof(bg::FlatOp));
-    memcpy(out->blob.data() + out->off_quad, quad.data(), quad.size() * sizeof(uint32_t));
-    memcpy(out->blob.data() + out->off_beg, beg, sizeof(beg));
-    memcpy(out->blob.data() + out->off_ranges, ranges.data(), ranges.size() * sizeof(uint16_t));
+        for (int i = 0; i + len <= N - 1; ++i) out->tab.ranges[r++] = (uint16_t)(i | (i + len) << 8);
+    return true;
 }
 
 }  // namespace
@@ -57,7 +48,7 @@ bool bg_rt_make(int eb, int u, int n, int d, int s, RtHost* out)
 {
     if (d % s != 0 || (long)(n + (n - 1) * (n - 2) / 2 + n) * d * eb >= 65536) return false;   // 16-bit row offsets
     switch (n) {
-#define BG_CASE(N) case N: make_for<N>(eb, u, d, s, out); return true;
+#define BG_CASE(N) case N: return make_for<N>(eb, u, d, s, out);
         BG_CASE(4) BG_CASE(5) BG_CASE(6) BG_CASE(7) BG_CASE(8) BG_CASE(9) BG_CASE(10)
         BG_CASE(11) BG_CASE(12) BG_CASE(13) BG_CASE(14) BG_CASE(15) BG_CASE(16)
 #undef BG_CASE

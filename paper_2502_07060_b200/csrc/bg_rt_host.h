@@ -1,9 +1,7 @@
-// bg_rt_host.h -- host side of bg_rt_kernel (bg_rt.cuh): the tile layout of a run-time n and its schedule as a
-// packed table, built once per shape by bg_api.cu and copied to the device it is first used on.
+// bg_rt_host.h -- host side of bg_rt_kernel (bg_rt.cuh): the tile layout of a run-time n and its schedule, built
+// once per shape by bg_api.cu and passed to every launch in the kernel's parameter block (bg::RtTables).
 #pragma once
 #include <stddef.h>
-
-#include <vector>
 
 #include "bg_common.cuh"
 
@@ -12,8 +10,7 @@ struct RtHost {
     int s;                         // lanes per point
     int threads, points_per_block;
     size_t smem;                   // dynamic shared memory per block
-    std::vector<unsigned char> blob;   // FlatOp[nops] | quad[] | beg[W+1] | ranges[r], each 16-byte aligned
-    size_t off_quad, off_beg, off_ranges;
+    bg::RtTables tab;              // ops, 4-gluon-split table, warp bounds, ranges
 };
 
 // layout and tables for elements of `eb` bytes moved in vector units of `u` elements, n gluons, d dimensions, s lanes

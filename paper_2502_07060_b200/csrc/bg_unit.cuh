@@ -32,16 +32,6 @@ constexpr uint32_t OP_GATHER = 32u;   // finisher of a shared current: check the
 constexpr uint32_t OP_LEND = 64u;     // block barrier after the op (end of the level)
 constexpr uint32_t OP_TOP = 128u;     // the current is J(1..m): amplitude instead of propagator and store
 
-struct FlatOp {
-    uint32_t ab;       // row A | row B << 16      (byte offsets in the lane's vector record)
-    uint32_t pso;      // row PS2_k | own row << 16
-    uint32_t u, v;     // U_A, V_B                 (byte offsets from the lane's scalar base)
-    uint32_t w;        // ci * m + j - 1 (position in the caller's `currents` array) | own row << 8 | level << 16
-                       // | OP_PART: first parked flag of the slot (word index) << 20
-    uint32_t lh;       // rows PS2_{i-1} | PS2_j << 16
-    uint32_t qcf;      // first entry of the op's 4-gluon splits in quad[] | c4 << 16 | flags << 24
-    uint32_t aux;      // OP_PART: scratch slot (byte offset from the first slot) ; OP_GATHER: mask of slots
-};
 
 // what the operand offsets of an op depend on besides n: element size, tile width and the start of the PS2 rows
 // and of the U / V tables
