@@ -116,12 +116,12 @@ int fill_general(int field, int metric, int n, int d, Launch* L)
     return BG_OK;
 }
 
-const void* rt_ptr(int field, int metric, int d, int s)
+const void* rt_ptr(int field, int metric, int d, int s, int w)
 {
     switch (field) {
-        case BG_FIELD_FP31: return bg_rt_kernel_ptr_fp31(metric, d, s);
-        case BG_FIELD_C128: return bg_rt_kernel_ptr_c128(metric, d, s);
-        case BG_FIELD_FPMONT: return bg_rt_kernel_ptr_mont(metric, d, s);
+        case BG_FIELD_FP31: return bg_rt_kernel_ptr_fp31(metric, d, s, w);
+        case BG_FIELD_C128: return bg_rt_kernel_ptr_c128(metric, d, s, w);
+        case BG_FIELD_FPMONT: return bg_rt_kernel_ptr_mont(metric, d, s, w);
     }
     return nullptr;
 }
@@ -134,7 +134,7 @@ int fill_rt(int field, int metric, int n, int d, Launch* L)
     for (int pass = 0; pass < 2; ++pass) {
         const int s = pass == 0 ? first : 3 - first;
         if (d % s != 0) continue;
-        const void* fn = rt_ptr(field, metric, d, s);
+        const void* fn = rt_ptr(field, metric, d, s, bg_rt_warps(n));
         if (!fn) continue;
         RtHost* h = new RtHost();
         if (!bg_rt_make(elem_bytes(field), vec_width(field, d), n, d, s, h) || h->smem > (size_t)kMaxSmemPerBlock) {

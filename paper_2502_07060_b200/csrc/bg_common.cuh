@@ -64,7 +64,7 @@ struct FlatOp {
 
 // bg_rt_kernel: the schedule of a run-time n travels with the launch as a kernel PARAMETER (constant bank: the ops
 // are read with uniform loads like the __constant__ tables of the compiled kernels; nothing is allocated or copied
-// to the device).  Sized for n = 16 with kRtWarps = 8 warps; 29 KB of the 32 KB a kernel may take.
+// to the device).  sized for n = 16 with 8 warps; 29 KB of the 32 KB a kernel may take.
 constexpr int kRtMaxOps = 680, kRtMaxQuad = 1820, kRtMaxRanges = 104;
 struct RtTables {
     FlatOp ops[kRtMaxOps];

@@ -33,12 +33,12 @@ BG_ENTRY_TABLES(BG_DECLARE_TABLE)
 
 // bg_general_kernel<F, MET, D> for d = 4..16, one translation unit per field (bg_inst_general_*.cu);
 // NULL if (metric, d) is out of range
-// bg_rt_kernel<F, MET, D, kRtWarps, S> for d = 4..16, S = 1 or (even d) 2, one translation unit per field
-// (bg_inst_rt_*.cu); NULL if out of range
-constexpr int kRtWarps = 8;
-const void* bg_rt_kernel_ptr_fp31(int metric, int d, int s);
-const void* bg_rt_kernel_ptr_c128(int metric, int d, int s);
-const void* bg_rt_kernel_ptr_mont(int metric, int d, int s);
+// bg_rt_kernel<F, MET, D, W, S> for d = 4..16, W = 4 or 8 warps per tile, S = 1 or (even d) 2, one translation unit per
+// field (bg_inst_rt_*.cu); NULL if out of range
+inline int bg_rt_warps(int n) { return n <= 8 ? 4 : 8; }     // as the compiled instances (measured at cfg2, cfg3)
+const void* bg_rt_kernel_ptr_fp31(int metric, int d, int s, int w);
+const void* bg_rt_kernel_ptr_c128(int metric, int d, int s, int w);
+const void* bg_rt_kernel_ptr_mont(int metric, int d, int s, int w);
 const void* bg_general_kernel_ptr_fp31(int metric, int d);
 const void* bg_general_kernel_ptr_c128(int metric, int d);
 const void* bg_general_kernel_ptr_mont(int metric, int d);

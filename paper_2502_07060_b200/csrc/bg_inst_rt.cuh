@@ -1,5 +1,5 @@
-// bg_inst_rt.cuh -- bg_rt_kernel<F, MET, D, W, S> for d = 4..16 of one (field, metric) pair (W = kRtWarps warps per
-// tile; S = 1 lane per point for every d, S = 2 for even d)
+// bg_inst_rt.cuh -- bg_rt_kernel<F, MET, D, W, S> for d = 4..16 of one (field, metric) pair (W = 4 or 8 warps per
+// tile, chosen by n: bg_rt_warps(); S = 1 lane per point for every d, S = 2 for even d)
 #pragma once
 #include "../../include/bg.h"
 #include "bg_entries.h"
@@ -7,33 +7,26 @@
 
 namespace {
 
-template <class F, int MET, int D>
+template <class F, int MET, int D, int W>
 const void* rt_for_s(int s)
 {
-    if (s == 1) return reinterpret_cast<const void*>(&bg::bg_rt_kernel<F, MET, D, kRtWarps, 1>);
+    if (s == 1) return reinterpret_cast<const void*>(&bg::bg_rt_kernel<F, MET, D, W, 1>);
     if constexpr (D % 2 == 0) {
-        if (s == 2) return reinterpret_cast<const void*>(&bg::bg_rt_kernel<F, MET, D, kRtWarps, 2>);
+        if (s == 2) return reinterpret_cast<const void*>(&bg::bg_rt_kernel<F, MET, D, W, 2>);
     }
     return nullptr;
 }
 
 template <class F, int MET>
-const void* rt_for_d(int d, int s)
+const void* rt_for_d(int d, int s, int w)
 {
     switch (d) {
-#define BG_CASE(D) case D: return rt_for_s<F, MET, D>(s);
+#define BG_CASE(D) case D: return w == 4 ? rt_for_s<F, MET, D, 4>(s) : w == 8 ? rt_for_s<F, MET, D, 8>(s) : nullptr;
         BG_CASE(4) BG_CASE(5) BG_CASE(6) BG_CASE(7) BG_CASE(8) BG_CASE(9) BG_CASE(10)
         BG_CASE(11) BG_CASE(12) BG_CASE(13) BG_CASE(14) BG_CASE(15) BG_CASE(16)
 #undef BG_CASE
     }
     return nullptr;
-}
-
-template <class F>
-const void* rt_for(int metric, int d, int s)
-{
-    return metric == BG_METRIC_MOSTLY_MINUS ? rt_for_d<F, BG_METRIC_MOSTLY_MINUS>(d, s)
-         : metric == BG_METRIC_ALTERNATING ? rt_for_d<F, BG_METRIC_ALTERNATING>(d, s) : nullptr;
 }
 
 }  // namespace

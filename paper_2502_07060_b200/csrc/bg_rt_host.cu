@@ -10,10 +10,10 @@
 
 namespace {
 
-template <int N>
+template <int N, int W>
 bool make_for(int eb, int u, int d, int s, RtHost* out)
 {
-    constexpr int W = kRtWarps, M = N - 1, R = M * (M - 1) / 2 - 1;
+    constexpr int M = N - 1, R = M * (M - 1) / 2 - 1;
     const bg::LevelProgram<N, W> p = bg::make_level_program<N, W>();
     const int tp = 32 / s;
     bg::RtLayout& L = out->lay;
@@ -48,7 +48,7 @@ bool bg_rt_make(int eb, int u, int n, int d, int s, RtHost* out)
 {
     if (d % s != 0 || (long)(n + (n - 1) * (n - 2) / 2 + n) * d * eb >= 65536) return false;   // 16-bit row offsets
     switch (n) {
-#define BG_CASE(N) case N: return make_for<N>(eb, u, d, s, out);
+#define BG_CASE(N) case N: return make_for<N, (N <= 8 ? 4 : 8)>(eb, u, d, s, out);   // bg_rt_warps(n)
         BG_CASE(4) BG_CASE(5) BG_CASE(6) BG_CASE(7) BG_CASE(8) BG_CASE(9) BG_CASE(10)
         BG_CASE(11) BG_CASE(12) BG_CASE(13) BG_CASE(14) BG_CASE(15) BG_CASE(16)
 #undef BG_CASE

@@ -250,11 +250,11 @@ VARIANTS = [("fp31", 8, 6, "unit1", 4), ("fp31", 8, 6, "unit1", 6), ("fp31", 8, 
             ("fp31", 9, 6, "unit1", 4), ("fp31", 6, 8, "unit1", 2), ("fp31", 8, 8, "unit1", 4), ("fp31", 9, 8, "unit1", 4),
             ("fp31", 6, 10, "unit1", 2), ("fp31", 9, 10, "unit1", 4), ("fp31", 5, 4, "unit1", 1), ("fp31", 7, 4, "unit1", 4),
             ("fp31", 10, 4, "unit1", 8), ("fp31", 4, 8, "unit1", 1), ("fp31", 5, 8, "unit1", 1), ("fp31", 7, 8, "unit1", 4),
-            # the tiled kernel for a run-time n (bg_rt_kernel): shapes with and without a compiled instance, one
-            # and two lanes per point, odd d
-            ("fp31", 8, 6, "rt", 8), ("fp31", 4, 4, "rt", 8), ("fp31", 13, 5, "rt", 8), ("fp31", 16, 4, "rt", 8),
-            ("fp31", 5, 16, "rt", 8), ("fp31", 11, 9, "rt", 8), ("fp31", 16, 16, "rt", 8),
-            ("c128", 6, 4, "rt", 8), ("c128", 12, 6, "rt", 8), ("c128", 7, 5, "rt", 8), ("c128", 13, 4, "rt", 8)]
+            # the tiled kernel for a run-time n (bg_rt_kernel; 4 warps per tile for n <= 8, else 8): shapes with and
+            # without a compiled instance, one and two lanes per point, odd d
+            ("fp31", 8, 6, "rt", 4), ("fp31", 4, 4, "rt", 4), ("fp31", 13, 5, "rt", 8), ("fp31", 16, 4, "rt", 8),
+            ("fp31", 5, 16, "rt", 4), ("fp31", 11, 9, "rt", 8), ("fp31", 16, 16, "rt", 8),
+            ("c128", 6, 4, "rt", 4), ("c128", 12, 6, "rt", 8), ("c128", 7, 5, "rt", 4), ("c128", 13, 4, "rt", 8)]
 KIND_ID = {"general": 0, "unit1": 1, "unit2": 2, "reg": 3, "rt": 4}
 
 
