@@ -9,7 +9,7 @@ BG_DEFINE_TABLE(cgrid0,
     unit_entry<C128, MM, 4, 6, 2, 2>(),
     unit_entry<C128, MM, 6, 6, 4, 2>(),
     unit_entry<C128, MM, 8, 6, 4, 2>(),
-    unit_entry<C128, MM, 10, 6, 8, 2>(),
+    unit_entry<C128, MM, 10, 6, 6, 2>(),      // 6 warps: two 115 KB tiles per SM (8 warps: 117 KB, one tile; 0.36 -> 0.51 of the DFMA peak)
     unit_entry<C128, MM, 5, 8, 2, 2>(),
     unit_entry<C128, MM, 7, 8, 4, 2>(),
     unit_entry<C128, MM, 9, 8, 8, 2>(),

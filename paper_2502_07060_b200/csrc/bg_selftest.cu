@@ -104,5 +104,6 @@ extern "C" int bg_selftest_schedules(void)
     if ((rc = check_level_program<12, 12>())) return rc - 200000;
     if ((rc = check_level_program<8, 3>())) return rc - 210000;
     if ((rc = check_level_program<16, 16>())) return rc - 220000;
+    if ((rc = check_level_program<10, 6>())) return rc - 230000;
     return rc;
 }
