@@ -240,8 +240,9 @@ int bg_set_kernel_override(int kind, int warps);
 /* Host-side self-check of the compile-time work schedules of the tiled kernels (every splitting
  * of Eq.(6), executed exactly once; a current shared between warps finished by the owner
  * of its first units as that warp's last task, every other part parked once in a scratch slot of its
- * own as its warp's first task and added exactly once).  Needs no GPU.  Returns 0, or a negative code
- * naming the first violated rule. */
+ * own as its warp's first task and added exactly once), and of the schedules the host builds at run time
+ * for shapes without a compiled instance (equal to the compiled ones on compiled shapes).  Needs no GPU.
+ * Returns 0, or a negative code naming the first violated rule. */
 int bg_selftest_schedules(void);
 
 /* ---- measurement support ---------------------------------------------------------------- */

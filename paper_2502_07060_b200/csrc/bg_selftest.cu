@@ -10,8 +10,12 @@
 // Pure host code: callable without a GPU (tests/test_abi.py).
 #include <stdint.h>
 
+#include <string.h>
+
 #include "../../include/bg.h"
+#include "bg_rt_host.h"
 #include "bg_schedule.cuh"
+#include "bg_unit.cuh"
 
 namespace {
 
@@ -76,6 +80,25 @@ int check_level_program()
     return 0;
 }
 
+// the schedule the host builds at run time for bg_rt_kernel (bg_rt_host.cu) against the one the compiler evaluated
+// for the compiled instance of the same shape: same ops, same 4-gluon-split table, same warp bounds, same layout
+template <class F, int N, int D, int W, int S>
+int check_rt_tables()
+{
+    typedef TileCfg<F, N, D, W, S, false> C;
+    static const FlatProgram<N, W> fp = make_flat_program<F, N, D, W, S>();
+    static RtHost h;
+    if (!bg_rt_make((int)sizeof(typename F::E), C::U, N, D, S, &h)) return -1;
+    if (h.lay.n != N || h.lay.ps0 != C::PS0 || h.lay.vstride != C::VSTRIDE || h.lay.sc_v != C::SC_V ||
+        h.lay.sc_w != C::SC_W || h.lay.sc_scr != C::SC_SCR || h.lay.nscal != C::NSCAL || h.lay.nslots != C::NSLOTS ||
+        h.smem != C::SMEM_BYTES || h.threads != 32 * W || h.points_per_block != C::TP)
+        return -2;
+    if (memcmp(h.tab.ops, fp.op, sizeof(fp.op)) != 0) return -3;
+    if (FlatProgram<N, W>::NQUAD > 0 && memcmp(h.tab.quad, fp.quad, sizeof(uint32_t) * FlatProgram<N, W>::NQUAD) != 0) return -4;
+    if (memcmp(h.tab.beg, fp.beg, sizeof(fp.beg)) != 0) return -5;
+    return 0;
+}
+
 }  // namespace
 
 extern "C" int bg_selftest_schedules(void)
@@ -105,5 +128,10 @@ extern "C" int bg_selftest_schedules(void)
     if ((rc = check_level_program<8, 3>())) return rc - 210000;
     if ((rc = check_level_program<16, 16>())) return rc - 220000;
     if ((rc = check_level_program<10, 6>())) return rc - 230000;
+    // bg_rt_make picks 4 warps per tile for n <= 8 and 8 above (bg_rt_warps): shapes whose compiled instance agrees
+    if ((rc = check_rt_tables<bg::Fp31, 8, 6, 4, 1>())) return rc - 300000;
+    if ((rc = check_rt_tables<bg::Fp31, 10, 8, 8, 1>())) return rc - 310000;
+    if ((rc = check_rt_tables<bg::Fp31, 12, 6, 8, 1>())) return rc - 320000;
+    if ((rc = check_rt_tables<bg::C128, 9, 6, 8, 2>())) return rc - 330000;
     return rc;
 }
