@@ -288,7 +288,7 @@ def _perms(n, K, seed):
     return np.array(out[:max(K, n + 2)], dtype=np.uint8)
 
 
-@pytest.mark.parametrize("n,d,batch", [(8, 6, 70), (6, 4, 133), (12, 6, 33), (7, 5, 45), (5, 7, 40)], ids=lambda v: str(v))
+@pytest.mark.parametrize("n,d,batch", [(8, 6, 70), (6, 4, 133), (12, 6, 33), (7, 5, 45), (5, 7, 40), (11, 7, 20)], ids=lambda v: str(v))
 def test_orderings_fp(bgl, oracle_mod, n, d, batch):
     import torch
     perms = _perms(n, 24, n)
