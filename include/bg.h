@@ -74,7 +74,8 @@ typedef enum {
     BG_OK = 0,
     BG_ERR_ARG = -1,          /* bad n, d, batch, field, metric, prime, null or misaligned pointer */
     BG_ERR_UNSUPPORTED = -2,  /* (field, n, d) needs more shared memory per point than an SM has */
-    BG_ERR_CUDA = -3          /* a CUDA runtime call or launch failed */
+    BG_ERR_CUDA = -3,         /* a CUDA runtime call or launch failed */
+    BG_ERR_TOO_LARGE = -4     /* bg_amplitudes_host_noalloc: batch > bg_noalloc_max_batch(field, n, d) */
 } bg_status_t;
 
 /* ---- the hot path (SURVEY.md §8(a) rows a0-a6 in ONE kernel launch) ------------------- */
@@ -187,6 +188,33 @@ int bg_amplitudes_host(int field, int n, int d, int64_t batch,
                        void* host_out, uint32_t* host_status,
                        void* workspace, size_t workspace_bytes);
 size_t bg_host_workspace_bytes(int field, int n, int d, int64_t chunk_points);
+
+/* The same call for a caller that CANNOT ALLOCATE device memory -- a plug-in beside a framework whose
+ * caching allocator already holds nearly all of HBM (its own cudaMalloc fails), a caller that must not pay
+ * cudaMalloc / cudaFree's device-wide synchronisation, or a plain C / Fortran program that owns host arrays
+ * only.  Such a caller has no `workspace` to pass to bg_amplitudes_host.  Here the device staging area is a
+ * fixed array of BG_NOALLOC_SCRATCH_BYTES inside the library image (a file-scope __device__ array): the CUDA
+ * runtime reserves it on every GPU that loads libbg_b200.so and keeps it until the process exits, whether
+ * or not this entry point is ever called.  The call allocates nothing (no cudaMalloc / cudaFree /
+ * cudaMallocAsync, no stream or event creation): H2D copies, ONE launch of the kernel bg_amplitudes_status
+ * would launch, D2H copies, all on `stream`, then it waits for `stream` and returns.
+ *   arguments  as bg_amplitudes_host: HOST arrays momenta, polarisations [batch][n][d], out [batch],
+ *              status NULL or [batch]; field BG_FIELD_FP31 or BG_FIELD_C128; mostly-minus metric.
+ *              Pageable host memory works, pinned memory is faster.
+ *   limit      one call takes at most bg_noalloc_max_batch(field, n, d) points (21 398 for n = 8, d = 6 over
+ *              F_p); a larger batch returns BG_ERR_TOO_LARGE before anything is copied or launched -- call
+ *              again with the next slice.  Nothing is chunked internally.
+ *   first call the first call on each device (with that device current) looks up the device address of the
+ *              array (cudaGetSymbolAddress); make that call before any stream capture begins.
+ *   sharing    every call on a device uses the same array.  Calls whose GPU work can overlap (two host threads,
+ *              two streams) race on it and return garbage: serialise them.  The array keeps the previous
+ *              call's bytes; a call reads back only what it has written itself, so nothing is cleared. */
+#define BG_NOALLOC_SCRATCH_BYTES (8u << 20)
+int bg_amplitudes_host_noalloc(int field, int n, int d, int64_t batch,
+                               const void* host_momenta, const void* host_polarisations,
+                               void* host_out, uint32_t* host_status, cudaStream_t stream);
+int64_t bg_noalloc_max_batch(int field, int n, int d);   /* 0 for an invalid (field, n, d) */
+size_t bg_noalloc_scratch_bytes(void);                   /* BG_NOALLOC_SCRATCH_BYTES of the loaded library */
 
 /* ---- introspection --------------------------------------------------------------------- */
 

@@ -20,13 +20,14 @@ FIELD_FP31, FIELD_C128, FIELD_FPMONT = 0, 1, 2
 METRIC_MOSTLY_MINUS, METRIC_ALTERNATING = 0, 1
 MAX_PRIMES = 8
 KERNEL_KINDS = {"default": -1, "general": 0, "unit1": 1, "unit2": 2, "reg": 3, "rt": 4}
-BG_OK, BG_ERR_ARG, BG_ERR_UNSUPPORTED, BG_ERR_CUDA = 0, -1, -2, -3
+BG_OK, BG_ERR_ARG, BG_ERR_UNSUPPORTED, BG_ERR_CUDA, BG_ERR_TOO_LARGE = 0, -1, -2, -3, -4
 PEAK_KINDS = {"imad_wide": 0, "imad": 1, "alu": 2, "mix": 3, "modmul": 4, "dfma": 5,
               "lds32": 6, "lds64": 7, "lds128": 8, "mix2": 9, "mix3": 10, "imad_wide_rz": 11}
 P31 = (1 << 31) - 1
 
 EXPORTS = ["bg_amplitudes", "bg_amplitudes_status", "bg_currents", "bg_evaluate", "bg_amplitudes_states",
-           "bg_amplitudes_primes", "bg_amplitudes_orderings", "bg_state_sum", "bg_states", "bg_generate", "bg_amplitudes_host", "bg_host_workspace_bytes", "bg_modulus",
+           "bg_amplitudes_primes", "bg_amplitudes_orderings", "bg_state_sum", "bg_states", "bg_generate", "bg_amplitudes_host", "bg_host_workspace_bytes",
+           "bg_amplitudes_host_noalloc", "bg_noalloc_max_batch", "bg_noalloc_scratch_bytes", "bg_modulus",
            "bg_status_string", "bg_version", "bg_op_count", "bg_kernel_info", "bg_kernel_info_problem",
            "bg_set_kernel_override", "bg_peak_probe", "bg_selftest_schedules"]
 
@@ -102,6 +103,11 @@ def load(rebuild_if_stale: bool = False):
     lib.bg_amplitudes_host.argtypes = [ci, ci, ci, i64, vp, vp, vp, vp, vp, sz]
     lib.bg_host_workspace_bytes.argtypes = [ci, ci, ci, i64]
     lib.bg_host_workspace_bytes.restype = sz
+    lib.bg_amplitudes_host_noalloc.argtypes = [ci, ci, ci, i64, vp, vp, vp, vp, vp]
+    lib.bg_amplitudes_host_noalloc.restype = ci
+    lib.bg_noalloc_max_batch.argtypes = [ci, ci, ci]
+    lib.bg_noalloc_max_batch.restype = i64
+    lib.bg_noalloc_scratch_bytes.restype = sz
     lib.bg_modulus.restype = ctypes.c_uint32
     lib.bg_status_string.argtypes = [ci]
     lib.bg_status_string.restype = ctypes.c_char_p
@@ -201,6 +207,20 @@ def bg_amplitudes_host(field, n, d, batch, host_mom_ptr, host_pol_ptr, host_out_
 
 def bg_host_workspace_bytes(field, n, d, chunk_points):
     return int(load().bg_host_workspace_bytes(field, n, d, chunk_points))
+
+
+def bg_amplitudes_host_noalloc(field, n, d, batch, host_mom_ptr, host_pol_ptr, host_out_ptr, host_status_ptr,
+                               stream_ptr=0):
+    return load().bg_amplitudes_host_noalloc(field, n, d, batch, host_mom_ptr, host_pol_ptr, host_out_ptr,
+                                             host_status_ptr, stream_ptr)
+
+
+def bg_noalloc_max_batch(field, n, d):
+    return int(load().bg_noalloc_max_batch(field, n, d))
+
+
+def bg_noalloc_scratch_bytes():
+    return int(load().bg_noalloc_scratch_bytes())
 
 
 def bg_modulus():
@@ -394,6 +414,23 @@ def currents(momenta, polarisations, stream=None):
         _check(bg_currents(field, n, d, batch, momenta.data_ptr(), polarisations.data_ptr(),
                            out.data_ptr(), cur.data_ptr(), status.data_ptr(), s))
     return out, cur, status
+
+
+def amplitudes_host_noalloc(momenta: np.ndarray, polarisations: np.ndarray, out=None, status=None, stream=None):
+    """bg_amplitudes_host_noalloc on HOST arrays: for a caller that cannot allocate device memory (the device
+    is already held by another framework's memory pool, or cudaMalloc's device-wide synchronisation is not
+    acceptable where the call is made).  Nothing is allocated on the device, not by this wrapper either: the
+    staging area is a fixed array inside the library, so the batch is limited to
+    bg_noalloc_max_batch(field, n, d) points per call (BgError "batch exceeds ..." beyond it) and calls that
+    overlap on the GPU race on that array.  Returns after the results are in `out` (and `status`)."""
+    field = FIELD_FP31 if momenta.dtype == np.uint32 else FIELD_C128
+    batch, n, d = momenta.shape
+    if out is None:
+        out = np.empty(batch, dtype=momenta.dtype)
+    s = 0 if stream is None else stream.cuda_stream
+    _check(bg_amplitudes_host_noalloc(field, n, d, batch, momenta.ctypes.data, polarisations.ctypes.data,
+                                      out.ctypes.data, None if status is None else status.ctypes.data, s))
+    return out
 
 
 def amplitudes_host(momenta: np.ndarray, polarisations: np.ndarray, workspace=None, out=None,

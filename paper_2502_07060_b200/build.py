@@ -16,7 +16,7 @@ SOURCES = ["bg_api.cu", "bg_rt_host.cu", "bg_inst_default.cu", "bg_inst_fp_alt.c
            "bg_inst_grid0.cu", "bg_inst_grid1.cu", "bg_inst_grid2.cu", "bg_inst_grid3.cu", "bg_inst_cgrid0.cu", "bg_inst_cgrid1.cu",
            "bg_inst_metric.cu", "bg_inst_mont.cu", "bg_inst_general_fp31.cu", "bg_inst_general_c128.cu",
            "bg_inst_general_mont.cu", "bg_inst_rt_fp31_mm.cu", "bg_inst_rt_fp31_alt.cu", "bg_inst_rt_c128_mm.cu", "bg_inst_rt_c128_alt.cu",
-           "bg_inst_rt_mont_mm.cu", "bg_inst_rt_mont_alt.cu", "bg_state_sum.cu", "bg_states.cu", "bg_generate.cu", "bg_peaks.cu", "bg_selftest.cu"]
+           "bg_inst_rt_mont_mm.cu", "bg_inst_rt_mont_alt.cu", "bg_state_sum.cu", "bg_states.cu", "bg_generate.cu", "bg_noalloc.cu", "bg_peaks.cu", "bg_selftest.cu"]
 HEADERS = ["bg_field.cuh", "bg_common.cuh", "bg_schedule.cuh", "bg_tile.cuh", "bg_unit.cuh", "bg_reg.cuh",
            "bg_general.cuh", "bg_rt.cuh", "bg_inst_rt.cuh", "bg_rt_host.h", "bg_entries.h", "bg_inst_common.cuh", "bg_inst_general.cuh", "bg_states.cuh", "bg_host_util.h"]
 

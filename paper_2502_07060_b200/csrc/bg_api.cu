@@ -591,6 +591,7 @@ const char* bg_status_string(int status)
         case BG_ERR_ARG: return "invalid argument";
         case BG_ERR_UNSUPPORTED: return "unsupported (field, n, d)";
         case BG_ERR_CUDA: return "CUDA error";
+        case BG_ERR_TOO_LARGE: return "batch exceeds bg_noalloc_max_batch (the fixed scratch array of the no-allocation entry point)";
     }
     return "unknown status";
 }
