@@ -324,12 +324,16 @@ def evaluate(momenta, polarisations, metric=METRIC_MOSTLY_MINUS, primes=(), stat
     (Eq.(5)).  Returns out [B] / [B,S] / [B,K] / [B,K,S] (leading [P] with primes)."""
     torch = _torch()
     ord_dev = None
+    launch = stream or torch.cuda.current_stream(momenta.device)
     if orderings is not None:
         o = np.ascontiguousarray(orderings, dtype=np.uint8)
         if o.ndim != 2 or o.shape[1] != momenta.shape[-2] or \
                 not (np.sort(o, axis=1) == np.arange(o.shape[1], dtype=np.uint8)).all():
             raise BgError("orderings must be [K, n] permutations of 0..n-1")
-        ord_dev = torch.from_numpy(o).to(momenta.device)
+        # the table is a temporary of this call: upload it ON the launch stream, so that the copy is ordered
+        # before the kernel and the caching allocator hands the block out again only in that stream's order
+        with torch.cuda.stream(launch):
+            ord_dev = torch.from_numpy(o).to(momenta.device)
     lead = 1 if primes else 0
     if momenta.dim() != 3 + lead or polarisations.dim() not in (3 + lead, 4 + lead):
         raise BgError("bad tensor ranks for evaluate()")
@@ -344,9 +348,10 @@ def evaluate(momenta, polarisations, metric=METRIC_MOSTLY_MINUS, primes=(), stat
     shape = ([len(primes)] if primes else []) + [batch] + ([ord_dev.shape[0]] if ord_dev is not None else []) + \
         ([states] if has_states else [])
     out = torch.empty(shape, dtype=momenta.dtype, device=momenta.device)
+    out.record_stream(launch)
     pb = problem(field, n, d, metric, states, tuple(primes), 0 if ord_dev is None else int(ord_dev.shape[0]),
                  None if ord_dev is None else ord_dev.data_ptr())
-    s = (stream or torch.cuda.current_stream(momenta.device)).cuda_stream
+    s = launch.cuda_stream
     with torch.cuda.device(momenta.device):
         _check(bg_evaluate(pb, batch, momenta.data_ptr(), polarisations.data_ptr(), out.data_ptr(), None,
                            None if status is None else status.data_ptr(), s))

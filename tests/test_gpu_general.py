@@ -310,6 +310,30 @@ def test_orderings_fp(bgl, oracle_mod, n, d, batch):
     assert not (g[:, 3:3 + n - 1].sum(axis=1) % P31).any()                               # U(1) decoupling
 
 
+def test_orderings_on_a_side_stream(bgl, oracle_mod):
+    """evaluate(orderings=..., stream=s) with s NOT torch's current stream: the permutation table is a temporary
+    of the call and must be uploaded on s (ordered before the kernel, its block reused only in s's order).  The
+    current stream is kept busy and churns the allocator meanwhile, which is what exposed the table to reuse."""
+    import torch
+    n, d, batch = 8, 6, 4000
+    perms = _perms(n, 24, n)
+    mom, pol, _ = inputs.make_fp_inputs(n, d, batch, seed=23)
+    dm, dp = bgl.to_device(mom), bgl.to_device(pol)
+    ref = oracle_mod.orderings(oracle_mod.FP31, mom[:300], pol[:300], perms, threads=8)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    for rep in range(5):
+        big = torch.empty(1 << 26, dtype=torch.uint8, device="cuda")
+        big.fill_(rep)                                             # long-running work on the current stream
+        out = bgl.evaluate(dm, dp, orderings=perms, stream=side)
+        junk = [torch.full((len(perms), n), 255, dtype=torch.uint8, device="cuda") for _ in range(8)]   # same size class
+        side.synchronize()
+        got = bgl.to_numpy(out)
+        assert np.array_equal(got[:300], ref), rep
+        del junk, big
+    torch.cuda.synchronize()
+
+
 def test_orderings_entry_point_states_and_complex(bgl, oracle_mod):
     import torch
     from oracle import rule
