@@ -38,7 +38,9 @@
  *   limits    4 <= n <= 16, 4 <= d <= 16 (the paper validates d = 4..10).
  *   memory    the caller owns every buffer; DEVICE pointers unless the name says host.
  *             Device pointers must be 16-byte aligned; out must not alias the inputs.
- *             The library allocates no device memory and keeps no per-call state.
+ *             The library allocates no device memory and keeps no per-call state; on the host a call
+ *             allocates nothing either (a shape's launch plan is built on its first use and cached; shapes
+ *             without a compiled instance stage their 29 KB schedule in a per-thread block).
  *   stream    launches are asynchronous on `stream`; nothing synchronises.
  *   errors    return value: BG_OK or a negative bg_status_t; nothing is thrown, nothing
  *             aborts.  Arguments are checked on the host before any launch.  batch == 0 is
@@ -115,7 +117,8 @@ typedef struct {
     int states;              /* S */
     int n_primes;
     uint32_t primes[BG_MAX_PRIMES];
-    int n_orderings;         /* K colour orderings per point (Eq.(5)); 0 or 1: the caller's order */
+    int n_orderings;         /* K colour orderings per point (Eq.(5)); 0 or 1: the caller's order.
+                                K <= 2^24 and max(K,1) * S < 2^27 (BG_ERR_ARG otherwise) */
     const unsigned char* orderings;   /* NULL, or DEVICE [K][n]: row o lists, for positions 1..n, which of the
                                 caller's legs (0-based) stands there; every row must be a permutation of
                                 0..n-1 (not checked: entries >= n are clamped to n-1) */
@@ -162,7 +165,8 @@ int bg_state_sum(int field, uint32_t prime, int64_t batch, int states, int trees
  * vector of Eq.(8)), eps and eps_tilde [count][d-2][d] (row x-1 = eps_x; eps~_1 = eps_2, eps~_2 = eps_1),
  * status NULL or [count] (bit0: a denominator of Eqs.(10),(16)-(18) vanished, the states are undefined).
  * 4 <= d <= 16.  prime: BG_FIELD_FPMONT only.  The mostly-minus spinors contain sqrt(-1): over F_p they
- * exist only for p = 1 mod 4 (BG_ERR_UNSUPPORTED otherwise, in particular for BG_FIELD_FP31); with
+ * exist only for p = 1 mod 4 (BG_ERR_UNSUPPORTED otherwise, in particular for BG_FIELD_FP31; also for a
+ * composite p with no quadratic non-residue below 256 -- primality stays the caller's job, the search is bounded); with
  * BG_METRIC_ALTERNATING they are rational.  Readings R13-R15 of DESIGN.md. */
 int bg_states(int field, uint32_t prime, int metric, int d, int64_t count, const void* momenta, const void* chi,
               void* eps, void* eps_tilde, uint32_t* status, cudaStream_t stream);

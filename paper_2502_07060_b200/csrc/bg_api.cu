@@ -41,7 +41,10 @@ struct Launch {
     // bg_rt_kernel: layout and schedule built by the host (kept for the life of the process); every launch
     // carries them in its parameter block
     RtHost* rt = nullptr;
+    uint64_t rt_id = 0;                // identifies the contents of *rt (the override path rebuilds it in place)
 };
+
+std::atomic<uint64_t> g_rt_ids{0};
 
 std::atomic<int> g_override_kind{-1};   // bg_kernel_info_t.specialised numbering; -1 = default
 std::atomic<int> g_override_w{0};
@@ -136,9 +139,12 @@ int fill_rt(int field, int metric, int n, int d, Launch* L)
         if (d % s != 0) continue;
         const void* fn = rt_ptr(field, metric, d, s, bg_rt_warps(n));
         if (!fn) continue;
-        RtHost* h = new RtHost();
+        // a cached Launch is filled once and keeps its RtHost for the life of the process; the one Launch of
+        // the override path is refilled when the override changes and reuses its RtHost
+        RtHost* h = L->rt ? L->rt : new RtHost();
+        memset(static_cast<void*>(h), 0, sizeof(RtHost));
         if (!bg_rt_make(elem_bytes(field), vec_width(field, d), n, d, s, h) || h->smem > (size_t)kMaxSmemPerBlock) {
-            delete h;
+            if (!L->rt) delete h;
             continue;
         }
         L->func = fn;
@@ -147,7 +153,8 @@ int fill_rt(int field, int metric, int n, int d, Launch* L)
         L->points_per_block = h->points_per_block;
         L->smem = (int)h->smem;
         L->stride = 0;
-        L->rt = h;                                              // (a Launch is filled once; never freed)
+        L->rt = h;
+        L->rt_id = ++g_rt_ids;
         return BG_OK;
     }
     return BG_ERR_UNSUPPORTED;
@@ -281,8 +288,12 @@ bool bg_spinor_consts_fp(uint32_t p, int metric, const bg::FpMont::Params* q, ui
         v = 1u;
     } else {
         if (p % 4u != 1u) return false;
-        uint64_t g = 2;                                   // a quadratic non-residue: g^((p-1)/2) = -1
-        while (powmod(g, (p - 1u) / 2u, p) != p - 1u) ++g;
+        // a quadratic non-residue: g^((p-1)/2) = -1.  For a prime the smallest one is tiny (half of all residues
+        // qualify); primality is the caller's job, so the search is bounded: a composite p for which no small g
+        // passes is refused instead of hanging the host
+        uint64_t g = 2;
+        while (g < 256 && powmod(g, (p - 1u) / 2u, p) != p - 1u) ++g;
+        if (g == 256) return false;
         m = v = powmod(g, (p - 1u) / 4u, p);              // sqrt(-1)
     }
     if (q) {                                              // to Montgomery form: x R mod p
@@ -340,14 +351,21 @@ int launch_typed(Launch* L, const bg_problem_t& pb, const typename F::Params& fl
     }
     const unsigned gy = pb.field == BG_FIELD_FPMONT ? (unsigned)pb.n_primes : 1u;
     bg::RtParams<F>* rp = nullptr;
-    if (L->kind == BG_KIND_RT) {                        // the schedule travels in the parameter block (29 KB)
-        rp = new bg::RtParams<F>;
-        rp->base = prm;
-        rp->tab = L->rt->tab;
+    if (L->kind == BG_KIND_RT) {
+        // the schedule travels in the parameter block (29 KB).  It is staged in a per-thread block that keeps the
+        // tables of the shape launched last: a repeated shape costs no allocation and no 29 KB copy, only `base`
+        // is patched (cudaLaunchKernel copies the parameters before it returns)
+        thread_local bg::RtParams<F> staged;
+        thread_local uint64_t staged_id = 0;
+        if (staged_id != L->rt_id) {
+            staged.tab = L->rt->tab;
+            staged_id = L->rt_id;
+        }
+        staged.base = prm;
+        rp = &staged;
     }
     void* args[] = {rp ? static_cast<void*>(rp) : static_cast<void*>(&prm)};
     const cudaError_t err = cudaLaunchKernel(L->func, dim3((unsigned)blocks, gy), dim3(L->threads), args, L->smem, stream);
-    delete rp;                                          // cudaLaunchKernel has copied the parameters
     if (err != cudaSuccess) {
         cudaGetLastError();
         return BG_ERR_CUDA;
@@ -362,6 +380,8 @@ int check_problem(const bg_problem_t* pb)
     if (rc != BG_OK) return rc;
     if (pb->states < 1 || pb->states > 65535) return BG_ERR_ARG;
     if (pb->n_orderings < 0 || pb->n_orderings > (1 << 24) || (pb->n_orderings > 1 && !pb->orderings)) return BG_ERR_ARG;
+    // the sweeps of one tile are numbered o * states + s (times 16 levels) in 32-bit arithmetic inside the kernels
+    if ((int64_t)(pb->n_orderings < 1 ? 1 : pb->n_orderings) * pb->states >= ((int64_t)1 << 27)) return BG_ERR_ARG;
     if (pb->field == BG_FIELD_FPMONT) {
         if (pb->n_primes < 1 || pb->n_primes > BG_MAX_PRIMES) return BG_ERR_ARG;
     } else if (pb->n_primes != 0) {

@@ -80,6 +80,71 @@ def test_kernel_info_and_bad_shapes(lib):
             binding.bg_kernel_info(*bad)
 
 
+def test_sweep_numbering_bound(lib):
+    """K orderings x S state configurations per point are numbered in 32-bit arithmetic inside the kernels (times 16
+    levels): the host refuses K * S >= 2^27 instead of letting the number overflow"""
+    fake = 4096                                                      # never dereferenced by the host-side checks
+    ok = binding.problem(0, 8, 6, states=4095, n_orderings=1 << 14, orderings_ptr=fake)      # K * S < 2^27
+    assert binding.bg_kernel_info_problem(ok)["specialised"] >= 1
+    with pytest.raises(binding.BgError):
+        binding.bg_kernel_info_problem(binding.problem(0, 8, 6, states=65535, n_orderings=1 << 12, orderings_ptr=fake))
+    with pytest.raises(binding.BgError):
+        binding.bg_kernel_info_problem(binding.problem(0, 8, 6, states=8, n_orderings=1 << 24, orderings_ptr=fake))
+
+
+@pytest.mark.timeout(120)
+def test_composite_modulus_is_refused_not_hung(lib):
+    """bg_states / bg_generate (mostly-minus metric, generic prime) need sqrt(-1) mod p and find it from a quadratic
+    non-residue.  Primality is the caller's job; for the composite 32771^2 = 1 mod 4 no small g passes Euler's
+    criterion, and the search must give up (BG_ERR_UNSUPPORTED) rather than spin on the host.  No launch happens."""
+    p = 32771 * 32771
+    assert (1 << 30) < p < (1 << 31) and p % 4 == 1
+    fake = 4096
+    rc = binding.bg_states(binding.FIELD_FPMONT, p, binding.METRIC_MOSTLY_MINUS, 4, 1, fake, fake + 256, fake + 512,
+                           fake + 1024)
+    assert rc == binding.BG_ERR_UNSUPPORTED
+    rc = binding.bg_generate(binding.FIELD_FPMONT, p, binding.METRIC_MOSTLY_MINUS, 4, 4, 1, 0, 0, (1, 1, -1, -1),
+                             fake, fake + 256)
+    assert rc == binding.BG_ERR_UNSUPPORTED
+
+
+DEFAULT_INSTANCES = [                                   # what cfg0, cfg2, cfg3, cfg4a, cfg4b and cfg1 launch by default
+    "bg::bg_unit_kernel<bg::Fp31, 0, 4, 4, 1, 1, false>", "bg::bg_unit_kernel<bg::Fp31, 0, 8, 6, 4, 1, false>",
+    "bg::bg_unit_kernel<bg::Fp31, 0, 10, 8, 8, 1, false>", "bg::bg_unit_kernel<bg::Fp31, 0, 12, 6, 8, 1, false>",
+    "bg::bg_unit_kernel<bg::C128, 0, 12, 6, 12, 2, false>", "bg::bg_reg_kernel<bg::C128, 0, 6, 4>"]
+
+
+def ptxas_entries():
+    """{demangled kernel name: (stack bytes, spill stores, spill loads, registers)} from the build's ptxas -v log"""
+    import shutil
+    import subprocess
+    log = os.path.join(build.CSRC, "ptxas.log")
+    if not os.path.exists(log) or not shutil.which("c++filt"):
+        pytest.skip("no ptxas.log (written by paper_2502_07060_b200.build) / c++filt")
+    ents = re.findall(r"Compiling entry function '(\S+)' for 'sm_100a'\nptxas info\s*: Function properties for \S+\n"
+                      r"\s*(\d+) bytes stack frame, (\d+) bytes spill stores, (\d+) bytes spill loads\n"
+                      r"ptxas info\s*: Used (\d+) registers", open(log).read())
+    names = subprocess.run(["c++filt"], input="\n".join(e[0] for e in ents), capture_output=True, text=True).stdout.split("\n")
+    clean = lambda nm: re.sub(r"\((int|bool)\)", "", re.sub(r"^void ", "", nm.split("(bg::BgParams")[0].split("(bg::RtParams")[0]))
+    return {clean(nm): tuple(int(x) for x in e[1:]) for nm, e in zip(names, ents)}
+
+
+def test_default_kernels_do_not_spill(lib):
+    """north_star asks for register spills as evidence: the six kernels the five configs launch by default keep
+    everything in registers (no stack frame, no spill bytes) -- guarded here the way the uniform datapath is below.
+    The instances that DO spill (none on a config's default path) are listed in DESIGN.md §6.6."""
+    ents = ptxas_entries()
+    assert len(ents) > 500
+    for name in DEFAULT_INSTANCES:
+        assert name in ents, (name, [k for k in ents if "8, 6, 4, 1" in k][:4])
+        stack, st, ld, regs = ents[name]
+        assert (stack, st, ld) == (0, 0, 0), (name, ents[name])
+        assert regs <= 255
+    # the run-time-n kernel over F_p (what shapes outside the compiled grid launch) may not spill more than a few words
+    worst = max((v[1] + v[2], k) for k, v in ents.items() if "bg_rt_kernel<bg::Fp31" in k or "bg_rt_kernel<bg::FpMont" in k)
+    assert worst[0] <= 64, worst
+
+
 def test_host_workspace_formula(lib):
     w = binding.bg_host_workspace_bytes(0, 8, 6, 1024)
     assert w == 2 * (2 * 1024 * 48 * 4 + 1024 * 4 + 1024 * 4)
