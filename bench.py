@@ -318,7 +318,7 @@ def r9_report(name: str, got, points: int) -> dict:
     return st
 
 
-def run_features(binding, torch, steps: int) -> list:
+def run_features(binding, torch, steps: int, sm_max_mhz: float | None = None) -> list:
     """SURVEY.md 8(f) rows, device-resident timings (inputs from the device generator)"""
     B = binding
     s = torch.cuda.current_stream().cuda_stream
@@ -331,8 +331,15 @@ def run_features(binding, torch, steps: int) -> list:
         if rc != B.BG_OK:
             raise RuntimeError(B.bg_status_string(rc))
 
+    def ok(rc):
+        # a BG_ERR_* return comes back in microseconds: it must stop the run, not become a huge points/s row
+        if rc != B.BG_OK:
+            raise RuntimeError(B.bg_status_string(rc))
+
     def row(name, amps, ms, **kw):
         rows.append({"feature": name, "value": amps / (ms * 1e-3), "unit": UNIT, "kernel_ms_median": ms, **kw})
+
+    clk_hz = (sm_max_mhz or 1965.0) * 1e6
 
     # f2: S state configurations per momentum point (Eq.(4)); the same 2^20 amplitudes per launch for every S
     for S in (1, 4, 16):
@@ -385,14 +392,14 @@ def run_features(binding, torch, steps: int) -> list:
         ms = time_device(torch, lambda: ev(pb, gb, mom, pol, outg), max(3, steps // 4))
         oc = op_counts("fp31", gn, gd)
         row(f"uncompiled shape (run-time-n tiled kernel): n={gn} d={gd} F_p, {gb} points", gb, ms,
-            roofline_frac=oc["mul_ref"] * gb / (ms * 1e-3) / (SM_COUNT * WIDE_MUL_LANES_PER_CLK_PER_SM * 1.965e9),
+            roofline_frac=oc["mul_ref"] * gb / (ms * 1e-3) / (SM_COUNT * WIDE_MUL_LANES_PER_CLK_PER_SM * clk_hz),
             kernel=B.bg_kernel_info(B.FIELD_FP31, gn, gd))
     # Eq.(4) state sum: HBM-bound
     T, S, bs = 2, 16, 1 << 20
     amps = [torch.randint(0, 2 ** 31 - 1, (bs, S), dtype=torch.int32, device="cuda") for _ in range(T)]
     outs = torch.empty(bs, dtype=torch.int32, device="cuda")
-    ms = time_device(torch, lambda: B.bg_state_sum(B.FIELD_FP31, 0, bs, S, [a.data_ptr() for a in amps],
-                                                   outs.data_ptr(), s), steps)
+    ms = time_device(torch, lambda: ok(B.bg_state_sum(B.FIELD_FP31, 0, bs, S, [a.data_ptr() for a in amps],
+                                                      outs.data_ptr(), s)), steps)
     rows.append({"feature": f"f2 state sum (Eq.(4)): {T} trees x S={S}, 2^20 points", "value": bs / (ms * 1e-3),
                  "unit": "points/s", "kernel_ms_median": ms, "hbm_GBs": (T * S + 1) * 4 * bs / (ms * 1e-3) / 1e9,
                  "hbm_frac": (T * S + 1) * 4 * bs / (ms * 1e-3) / 1e9 / hbm_peak()})
@@ -400,8 +407,8 @@ def run_features(binding, torch, steps: int) -> list:
     gb = 1 << 20
     mom = torch.empty((gb, n, d), dtype=torch.int32, device="cuda")
     pol = torch.empty_like(mom)
-    ms = time_device(torch, lambda: B.bg_generate(B.FIELD_FP31, 0, 0, n, d, gb, 0, 0, None, mom.data_ptr(),
-                                                  pol.data_ptr(), None, None, s), steps)
+    ms = time_device(torch, lambda: ok(B.bg_generate(B.FIELD_FP31, 0, 0, n, d, gb, 0, 0, None, mom.data_ptr(),
+                                                     pol.data_ptr(), None, None, s)), steps)
     rows.append({"feature": "f1 device generator: n=8 d=6 F_p, 2^20 points", "value": gb / (ms * 1e-3),
                  "unit": "points/s", "kernel_ms_median": ms, "hbm_frac": 2 * n * d * 4 * gb / (ms * 1e-3) / 1e9 / hbm_peak()})
     momA, _, refA, _ = B.generate(B.FIELD_FP31, n, d, 1 << 17, seed=0, metric=1, want_references=True)
@@ -409,8 +416,8 @@ def run_features(binding, torch, steps: int) -> list:
     kv, cv = momA.reshape(-1, d), chi.reshape(-1, 4).contiguous()
     eps = torch.empty((kv.shape[0], d - 2, d), dtype=torch.int32, device="cuda")
     til = torch.empty_like(eps)
-    ms = time_device(torch, lambda: B.bg_states(B.FIELD_FP31, 0, 1, d, kv.shape[0], kv.data_ptr(), cv.data_ptr(),
-                                                eps.data_ptr(), til.data_ptr(), None, s), steps)
+    ms = time_device(torch, lambda: ok(B.bg_states(B.FIELD_FP31, 0, 1, d, kv.shape[0], kv.data_ptr(), cv.data_ptr(),
+                                                   eps.data_ptr(), til.data_ptr(), None, s)), steps)
     rows.append({"feature": "f1 device states (Eqs.(8)-(18)): d=6 alternating metric F_p, 2^20 vectors",
                  "value": kv.shape[0] / (ms * 1e-3), "unit": "vectors/s", "kernel_ms_median": ms})
     return rows
@@ -613,7 +620,7 @@ def run_gpu(args) -> None:
                 per.append(entry)
                 del r
             line["per_config"] = per
-            line["features"] = run_features(binding, torch, args.config_steps)
+            line["features"] = run_features(binding, torch, args.config_steps, clocks.get("sm_max_mhz"))
             se = seeded_e2e(binding, torch, name, e2e_steps)
             se["matches_device_path"] = bool(np.array_equal(se.pop("result"), binding.to_numpy(res["out"]))) \
                 if cfg["field"] == "fp31" else None
