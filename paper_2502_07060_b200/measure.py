@@ -49,3 +49,36 @@ def measure_peaks(kinds=None, sms: int | None = None, target_ms: float = 3.0, re
         res[kind] = {"ops_per_s": ops * blocks * threads / (best * 1e-3),
                      "ms_best": best, "ms_median": statistics.median(ts), "iters": iters}
     return res
+
+
+def _main(argv=None) -> int:
+    """python -m paper_2502_07060_b200.measure [--once ITERS] [kind ...]
+
+    Prints the pipe-peak probes of this GPU as one JSON line (thread-operations per second per kind; kinds as in
+    binding.PEAK_KINDS, default all).  --once ITERS launches every named probe exactly once with that many loop
+    iterations and times nothing: the form to put under `ncu` when one wants the counters of a probe."""
+    import argparse
+    import json
+
+    import torch
+    ap = argparse.ArgumentParser(prog="python -m paper_2502_07060_b200.measure")
+    ap.add_argument("kinds", nargs="*", default=None)
+    ap.add_argument("--once", type=int, default=0, metavar="ITERS")
+    args = ap.parse_args(argv)
+    binding.load()
+    kinds = args.kinds or list(binding.PEAK_KINDS)
+    if args.once:
+        sms = torch.cuda.get_device_properties(0).multi_processor_count
+        blocks, threads = sms * 8, 256
+        sink = torch.zeros(blocks * threads, dtype=torch.int32, device="cuda")
+        s = torch.cuda.current_stream().cuda_stream
+        ops = {k: binding.bg_peak_probe(k, args.once, blocks, threads, sink.data_ptr(), s) for k in kinds}
+        torch.cuda.synchronize()
+        print(json.dumps({"once": args.once, "blocks": blocks, "threads": threads, "ops_per_thread": ops}))
+        return 0
+    print(json.dumps(measure_peaks(kinds)))
+    return 0
+
+
+if __name__ == "__main__":
+    raise SystemExit(_main())
