@@ -394,6 +394,19 @@ def run_features(binding, torch, steps: int, sm_max_mhz: float | None = None) ->
         row(f"uncompiled shape (run-time-n tiled kernel): n={gn} d={gd} F_p, {gb} points", gb, ms,
             roofline_frac=oc["mul_ref"] * gb / (ms * 1e-3) / (SM_COUNT * WIDE_MUL_LANES_PER_CLK_PER_SM * clk_hz),
             kernel=B.bg_kernel_info(B.FIELD_FP31, gn, gd))
+    # ... and with S = 4 state configurations per point (the MULTI instantiation of bg_rt_kernel; until round 3 this
+    # ran the one-thread-per-point fallback)
+    gn, gd, gb, gS = 13, 5, 1 << 13, 4
+    mom, pol0, _ = B.generate(B.FIELD_FP31, gn, gd, gb, seed=0)
+    pol = torch.stack([pol0] + [B.generate(B.FIELD_FP31, gn, gd, gb, seed=s_)[1] for s_ in range(1, gS)], dim=1).contiguous()
+    outg = torch.empty((gb, gS), dtype=torch.int32, device="cuda")
+    pb = B.problem(B.FIELD_FP31, gn, gd, states=gS)
+    ms = time_device(torch, lambda: ev(pb, gb, mom, pol, outg), max(3, steps // 4))
+    oc = op_counts("fp31", gn, gd)
+    row(f"uncompiled shape, S={gS} states (run-time-n tiled kernel): n={gn} d={gd} F_p, {gb} points", gb * gS, ms,
+        roofline_frac=oc["mul_ref"] * gb * gS / (ms * 1e-3) / (SM_COUNT * WIDE_MUL_LANES_PER_CLK_PER_SM * clk_hz),
+        kernel=B.bg_kernel_info_problem(pb))
+    del pol, pol0
     # Eq.(4) state sum: HBM-bound
     T, S, bs = 2, 16, 1 << 20
     amps = [torch.randint(0, 2 ** 31 - 1, (bs, S), dtype=torch.int32, device="cuda") for _ in range(T)]

@@ -119,31 +119,31 @@ int fill_general(int field, int metric, int n, int d, Launch* L)
     return BG_OK;
 }
 
-const void* rt_ptr(int field, int metric, int d, int s, int w)
+const void* rt_ptr(int field, int metric, int d, int s, int w, bool multi)
 {
     switch (field) {
-        case BG_FIELD_FP31: return bg_rt_kernel_ptr_fp31(metric, d, s, w);
-        case BG_FIELD_C128: return bg_rt_kernel_ptr_c128(metric, d, s, w);
-        case BG_FIELD_FPMONT: return bg_rt_kernel_ptr_mont(metric, d, s, w);
+        case BG_FIELD_FP31: return bg_rt_kernel_ptr_fp31(metric, d, s, w, multi);
+        case BG_FIELD_C128: return bg_rt_kernel_ptr_c128(metric, d, s, w, multi);
+        case BG_FIELD_FPMONT: return bg_rt_kernel_ptr_mont(metric, d, s, w, multi);
     }
     return nullptr;
 }
 
 // the tiled kernel for a run-time n: one lane per point if a 32-point tile fits shared memory (complex128: two
 // lanes per point first, as in the compiled tables), else two lanes per point, else not available
-int fill_rt(int field, int metric, int n, int d, Launch* L)
+int fill_rt(int field, int metric, int n, int d, bool multi, Launch* L)
 {
     const int first = field == BG_FIELD_C128 && d % 2 == 0 ? 2 : 1;
     for (int pass = 0; pass < 2; ++pass) {
         const int s = pass == 0 ? first : 3 - first;
         if (d % s != 0) continue;
-        const void* fn = rt_ptr(field, metric, d, s, bg_rt_warps(n));
+        const void* fn = rt_ptr(field, metric, d, s, bg_rt_warps(n), multi);
         if (!fn) continue;
         // a cached Launch is filled once and keeps its RtHost for the life of the process; the one Launch of
         // the override path is refilled when the override changes and reuses its RtHost
         RtHost* h = L->rt ? L->rt : new RtHost();
         memset(static_cast<void*>(h), 0, sizeof(RtHost));
-        if (!bg_rt_make(elem_bytes(field), vec_width(field, d), n, d, s, h) || h->smem > (size_t)kMaxSmemPerBlock) {
+        if (!bg_rt_make(elem_bytes(field), vec_width(field, d), n, d, s, multi, h) || h->smem > (size_t)kMaxSmemPerBlock) {
             if (!L->rt) delete h;
             continue;
         }
@@ -163,7 +163,7 @@ int fill_rt(int field, int metric, int n, int d, Launch* L)
 // run-time-n shapes: the tiled kernel where it applies, else one thread per point
 int fill_uncompiled(int field, int metric, int n, int d, bool multi_state, Launch* L)
 {
-    if (!multi_state && fill_rt(field, metric, n, d, L) == BG_OK) return BG_OK;
+    if (fill_rt(field, metric, n, d, multi_state, L) == BG_OK) return BG_OK;
     return fill_general(field, metric, n, d, L);
 }
 

@@ -36,9 +36,9 @@ BG_ENTRY_TABLES(BG_DECLARE_TABLE)
 // bg_rt_kernel<F, MET, D, W, S> for d = 4..16, W = 4 or 8 warps per tile, S = 1 or (even d) 2, one translation unit per
 // field (bg_inst_rt_*.cu); NULL if out of range
 inline int bg_rt_warps(int n) { return n <= 8 ? 4 : 8; }     // as the compiled instances (measured at cfg2, cfg3)
-const void* bg_rt_kernel_ptr_fp31(int metric, int d, int s, int w);
-const void* bg_rt_kernel_ptr_c128(int metric, int d, int s, int w);
-const void* bg_rt_kernel_ptr_mont(int metric, int d, int s, int w);
+const void* bg_rt_kernel_ptr_fp31(int metric, int d, int s, int w, bool multi);
+const void* bg_rt_kernel_ptr_c128(int metric, int d, int s, int w, bool multi);
+const void* bg_rt_kernel_ptr_mont(int metric, int d, int s, int w, bool multi);
 const void* bg_general_kernel_ptr_fp31(int metric, int d);
 const void* bg_general_kernel_ptr_c128(int metric, int d);
 const void* bg_general_kernel_ptr_mont(int metric, int d);

@@ -7,8 +7,10 @@
 // and program policies) -- but the layout and the ops are kernel ARGUMENTS: the host builds the schedule at the first
 // call for a shape (bg_rt_host.cu) and every launch carries it in its parameter block (RtParams, bg_common.cuh: the
 // constant bank, read with uniform loads like the compiled kernels' tables).  Only the per-tile setup (rows a0-a3) is
-// restated here with run-time row counts.  One state configuration and one colour ordering per point; requests
-// with more of either, and shapes whose 16-point tile does not fit shared memory, run bg_general_kernel.
+// restated here with run-time row counts.  The MULTI instantiation loops over K colour orderings and S state
+// configurations per point like bg_unit_kernel's (a1-a3 once per ordering, the sweep once per configuration; its
+// layout keeps -1/P^2 in a table of its own, because the propagators outlive a sweep); the plain one serves one
+// of each.  Shapes whose 16-point tile does not fit shared memory run bg_general_kernel.
 //
 // Round 2 ran every such shape on bg_general_kernel (one thread per point, at most one warp per block: 0.12 of the
 // multiplier peak at n = 13, d = 5 and n = 16, d = 4 against 0.6-0.7 for the compiled shapes).
@@ -41,23 +43,34 @@ struct RtLane {
 };
 
 // a0: stage `rows` rows of the tile's points into record rows [row0, row0 + rows), coalesced, one vector unit
-// per thread and step
+// per thread and step.  perm: NULL, or the colour ordering (Eq.(5)): record row row0 + i receives the
+// caller's row perm[i] (entries >= n are clamped, bg.h)
 template <class F, int D, int W>
 __device__ __forceinline__ void rt_stage(const F& f, typename F::E* vec, int vstride, int valid,
-                                         const typename F::E* src, long long pstride, int row0, int rows)
+                                         const typename F::E* src, long long pstride, int row0, int rows,
+                                         const unsigned char* __restrict__ perm = nullptr, int n = 0)
 {
     constexpr int U = VecWidth<F, D>::value, upr = D / U;
     typedef typename VecType<F, U>::type V;
     const int upp = rows * upr, total = valid * upp;
+    if (perm == nullptr) {
 #pragma unroll 4
-    for (int g = threadIdx.x; g < total; g += 32 * W) {
-        const int p = g / upp, u = g - p * upp;
-        V* r = reinterpret_cast<V*>(vec + (size_t)p * vstride) + row0 * upr;
-        r[u] = load_unit<F>(f, __ldg(reinterpret_cast<const V*>(src + p * pstride) + u));
+        for (int g = threadIdx.x; g < total; g += 32 * W) {
+            const int p = g / upp, u = g - p * upp;
+            V* r = reinterpret_cast<V*>(vec + (size_t)p * vstride) + row0 * upr;
+            r[u] = load_unit<F>(f, __ldg(reinterpret_cast<const V*>(src + p * pstride) + u));
+        }
+    } else {
+#pragma unroll 2
+        for (int g = threadIdx.x; g < total; g += 32 * W) {
+            const int p = g / upp, u = g - p * upp, row = u / upr, c = u - row * upr;
+            V* r = reinterpret_cast<V*>(vec + (size_t)p * vstride) + row0 * upr;
+            r[u] = load_unit<F>(f, __ldg(reinterpret_cast<const V*>(src + p * pstride) + min((int)__ldg(perm + row), n - 1) * upr + c));
+        }
     }
 }
 
-template <class F, int MET, int D, int W, int S>
+template <class F, int MET, int D, int W, int S, bool MULTI>
 __global__ void __launch_bounds__(32 * W) bg_rt_kernel(const __grid_constant__ RtParams<F> P)
 {
     const BgParams<F>& prm = P.base;
@@ -81,19 +94,49 @@ __global__ void __launch_bounds__(32 * W) bg_rt_kernel(const __grid_constant__ R
     const int valid = (int)min((long long)TP, prm.batch - tile0);
     t.pt = tile0 + point;
     t.live = point < valid;
+    const int states = MULTI ? prm.states : 1, n_ord = MULTI ? prm.n_orderings : 1;
     const long long pbase = (long long)blockIdx.y * prm.batch; // first point of this prime's arrays
+    const E* gmom = prm.mom + (pbase + tile0) * nd;
+    const E* gpol = prm.pol + (pbase + tile0) * states * nd;
+    E* gout = prm.out + (pbase + t.pt) * n_ord * states;
     E* recf = vec + (size_t)point * L.vstride;                 // the point's record, all components
     E* rec = recf + t.mu0;                                     // this lane's components
     E* sc = scal + point;
     uint32_t* gstat = prm.status ? prm.status + pbase : nullptr;
+    RtLay lay;
+    lay.l = L;
+    const RtProg prog{P.tab};
+
+    // single-gluon U = V = 2 k_c . eps_c (zero for transverse states; kept for any input, R4)
+    auto singles = [&]() {
+#pragma unroll 1
+        for (int c = warp + 1; c <= m; c += W) {
+            E lo[DL], hi[DL], k2[DL], e[DL];
+            ld_vec<F, DL>(rec + (PS0 + c - 1) * D, lo);
+            ld_vec<F, DL>(rec + (PS0 + c) * D, hi);
+            ld_vec<F, DL>(rec + (c - 1) * D, e);
+            lower_diff<F, MET, DL>(f, t.mu0, hi, lo, k2);                               // 2 * covariant k_c
+            sc[(c - 1) * TP] = lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, k2, e)));
+            if (prm.currents && t.live) {
+                E* dst = prm.currents + (t.pt * m * m + (long long)(c - 1) * m + (c - 1)) * D + t.mu0;
+#pragma unroll
+                for (int mu = 0; mu < DL; ++mu) dst[mu] = f.to_output(e[mu]);
+            }
+        }
+    };
 
     if (warp == 0 && lane < TP) stat[lane] = 0;
 #pragma unroll 1
     for (int sl = warp; sl < L.nslots; sl += W) stat[TP + 32 * sl + lane] = 0;
 
+#pragma unroll 1
+    for (int o = 0; o < n_ord; ++o, gout += states) {
+    // colour ordering o (Eq.(5)): the inputs are re-staged in that order, everything below runs unchanged
+    const unsigned char* perm = MULTI && prm.orderings ? prm.orderings + o * n : nullptr;
+    if (MULTI && o > 0) __syncthreads();                       // the previous sweep is done with the record
     // ---- a0: momenta k_1..k_m into the PS2 rows 1..m (summed in place below), eps_1..eps_n into rows [0, n) ----
-    rt_stage<F, D, W>(f, vec, L.vstride, valid, prm.mom + (pbase + tile0) * nd, nd, PS0 + 1, m);
-    rt_stage<F, D, W>(f, vec, L.vstride, valid, prm.pol + (pbase + tile0) * nd, nd, 0, n);
+    rt_stage<F, D, W>(f, vec, L.vstride, valid, gmom, nd, PS0 + 1, m, perm, n);
+    rt_stage<F, D, W>(f, vec, L.vstride, valid, gpol, (long long)states * nd, 0, n, perm, n);
     __syncthreads();
 
     // ---- a1: doubled prefix sums PS2_c = 2 (k_1 + .. + k_c)  (Eq.(7)), running sum by warp 0 ----
@@ -113,24 +156,11 @@ __global__ void __launch_bounds__(32 * W) bg_rt_kernel(const __grid_constant__ R
     }
     __syncthreads();
 
-    // ---- single-gluon U = V = 2 k_c . eps_c (zero for transverse states; kept for any input, R4) ----
-#pragma unroll 1
-    for (int c = warp + 1; c <= m; c += W) {
-        E lo[DL], hi[DL], k2[DL], e[DL];
-        ld_vec<F, DL>(rec + (PS0 + c - 1) * D, lo);
-        ld_vec<F, DL>(rec + (PS0 + c) * D, hi);
-        ld_vec<F, DL>(rec + (c - 1) * D, e);
-        lower_diff<F, MET, DL>(f, t.mu0, hi, lo, k2);                               // 2 * covariant k_c
-        sc[(c - 1) * TP] = lane_sum<F, S, TP>(f, f.reduce(dot_plain<F, DL>(f, k2, e)));
-        if (prm.currents && t.live) {
-            E* dst = prm.currents + (t.pt * m * m + (long long)(c - 1) * m + (c - 1)) * D + t.mu0;
-#pragma unroll
-            for (int mu = 0; mu < DL; ++mu) dst[mu] = f.to_output(e[mu]);
-        }
-    }
+    singles();                                                 // first state configuration
 
     // ---- a2 + a3: invariants 4 P_{i,j}^2 and -1/P^2 (the sign: bg_unit.cuh accumulates minus the bracket); the r
-    //      proper ranges are dealt round-robin to the W*S (half-)warps, each batch-inverts its share (zero-safe) ----
+    //      proper ranges are dealt round-robin to the W*S (half-)warps, each batch-inverts its share (zero-safe).
+    //      Momenta only: once per tile and ordering ----
     {
         constexpr int VW = W * S;
         const int vw = warp * S + t.half;
@@ -148,7 +178,7 @@ __global__ void __launch_bounds__(32 * W) bg_rt_kernel(const __grid_constant__ R
             Wt[r * TP] = f.canon(f.neg(f.reduce(dot_plain<F, D>(f, nx, x))));
         }
         if constexpr (F::kExact) {
-            E* tmp = sc + L.sc_v * TP;                         // prefix products, in the not-yet-used V slots
+            E* tmp = sc + L.sc_v * TP;                         // prefix products, in the V slots (dead until the sweep)
             E c = f.one();
 #pragma unroll 1
             for (int r = vw; r < L.r; r += VW) {
@@ -179,14 +209,22 @@ __global__ void __launch_bounds__(32 * W) bg_rt_kernel(const __grid_constant__ R
         if (gstat && status) atomicOr(&stat[point], status);
     }
     __syncthreads();
-    if (gstat && warp == 0 && t.half == 0 && t.live) gstat[t.pt] = stat[point];
+    if (gstat && warp == 0 && t.half == 0 && t.live) gstat[t.pt] = stat[point];   // (accumulates over the orderings)
 
-    // ---- a4-a6: the level sweep (bg_unit.cuh) ----
-    RtLay lay;
-    lay.l = L;
-    const RtProg prog{P.tab};
-    unit_sweep_body<F, MET, D, S>(f, lay, prog, t, warp, rec, sc, stat + TP + lane, 0u, prm.out + pbase + t.pt,
-                                  prm.currents);
+    // ---- a4-a6: the level sweep (bg_unit.cuh), once per state configuration (Eq.(4)) ----
+#pragma unroll 1
+    for (int s = 0; s < states; ++s) {
+        if (MULTI && s > 0) {
+            __syncthreads();                                   // the previous sweep is done with eps_n
+            rt_stage<F, D, W>(f, vec, L.vstride, valid, gpol + (long long)s * nd, (long long)states * nd, 0, n, perm, n);
+            __syncthreads();
+            singles();
+            __syncthreads();
+        }
+        unit_sweep_body<F, MET, D, S>(f, lay, prog, t, warp, rec, sc, stat + TP + lane,
+                                      ((uint32_t)o * (uint32_t)states + (uint32_t)s) * 16u, gout + s, prm.currents);
+    }
+    }
 }
 
 }  // namespace bg

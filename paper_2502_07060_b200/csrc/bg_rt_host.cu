@@ -11,7 +11,7 @@
 namespace {
 
 template <int N, int W>
-bool make_for(int eb, int u, int d, int s, RtHost* out)
+bool make_for(int eb, int u, int d, int s, bool multi, RtHost* out)
 {
     constexpr int M = N - 1, R = M * (M - 1) / 2 - 1;
     const bg::LevelProgram<N, W> p = bg::make_level_program<N, W>();
@@ -23,8 +23,8 @@ bool make_for(int eb, int u, int d, int s, RtHost* out)
     const int vec_units = (j_rows + M + 1) * d / u;            // odd number of vector units: conflict-free lanes
     L.vstride = (vec_units % 2 == 1 ? vec_units : vec_units + 1) * u;
     L.sc_v = j_rows;
-    L.sc_w = N;                                                // 1/P^2 parked in the U slots of the multi-gluon rows
-    L.sc_scr = j_rows + R;
+    L.sc_w = multi ? j_rows + R : N;                           // 1/P^2: a table of its own, or parked in the U slots of
+    L.sc_scr = j_rows + R + (multi ? R : 0);                   // the multi-gluon rows (as TileCfg's KW, bg_tile.cuh)
     L.nslots = p.nslots;
     L.nscal = L.sc_scr + L.nslots * (d + 1);
     out->s = s;
@@ -44,11 +44,11 @@ bool make_for(int eb, int u, int d, int s, RtHost* out)
 
 }  // namespace
 
-bool bg_rt_make(int eb, int u, int n, int d, int s, RtHost* out)
+bool bg_rt_make(int eb, int u, int n, int d, int s, bool multi, RtHost* out)
 {
     if (d % s != 0 || (long)(n + (n - 1) * (n - 2) / 2 + n) * d * eb >= 65536) return false;   // 16-bit row offsets
     switch (n) {
-#define BG_CASE(N) case N: return make_for<N, (N <= 8 ? 4 : 8)>(eb, u, d, s, out);   // bg_rt_warps(n)
+#define BG_CASE(N) case N: return make_for<N, (N <= 8 ? 4 : 8)>(eb, u, d, s, multi, out);   // bg_rt_warps(n)
         BG_CASE(4) BG_CASE(5) BG_CASE(6) BG_CASE(7) BG_CASE(8) BG_CASE(9) BG_CASE(10)
         BG_CASE(11) BG_CASE(12) BG_CASE(13) BG_CASE(14) BG_CASE(15) BG_CASE(16)
 #undef BG_CASE

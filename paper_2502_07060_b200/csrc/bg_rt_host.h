@@ -14,5 +14,7 @@ struct RtHost {
 };
 
 // layout and tables for elements of `eb` bytes moved in vector units of `u` elements, n gluons, d dimensions, s lanes
-// per point (d % s == 0); false if n is out of range.  The caller checks smem against the device limit.
-bool bg_rt_make(int eb, int u, int n, int d, int s, RtHost* out);
+// per point (d % s == 0); multi: the layout of the MULTI instantiation (-1/P^2 in a table of its own instead of the U
+// slots of the multi-gluon rows: with several orderings / state configurations per point the propagators outlive a
+// sweep).  false if n is out of range.  The caller checks smem against the device limit.
+bool bg_rt_make(int eb, int u, int n, int d, int s, bool multi, RtHost* out);

@@ -88,7 +88,7 @@ int check_rt_tables()
     typedef TileCfg<F, N, D, W, S, false> C;
     static const FlatProgram<N, W> fp = make_flat_program<F, N, D, W, S>();
     static RtHost h;
-    if (!bg_rt_make((int)sizeof(typename F::E), C::U, N, D, S, &h)) return -1;
+    if (!bg_rt_make((int)sizeof(typename F::E), C::U, N, D, S, false, &h)) return -1;
     if (h.lay.n != N || h.lay.ps0 != C::PS0 || h.lay.vstride != C::VSTRIDE || h.lay.sc_v != C::SC_V ||
         h.lay.sc_w != C::SC_W || h.lay.sc_scr != C::SC_SCR || h.lay.nscal != C::NSCAL || h.lay.nslots != C::NSLOTS ||
         h.smem != C::SMEM_BYTES || h.threads != 32 * W || h.points_per_block != C::TP)
@@ -96,6 +96,14 @@ int check_rt_tables()
     if (memcmp(h.tab.ops, fp.op, sizeof(fp.op)) != 0) return -3;
     if (FlatProgram<N, W>::NQUAD > 0 && memcmp(h.tab.quad, fp.quad, sizeof(uint32_t) * FlatProgram<N, W>::NQUAD) != 0) return -4;
     if (memcmp(h.tab.beg, fp.beg, sizeof(fp.beg)) != 0) return -5;
+    // the layout of the MULTI instantiation (propagator table of its own) against TileCfg's KW layout
+    typedef TileCfg<F, N, D, W, S, true> CK;
+    static RtHost hk;
+    if (!bg_rt_make((int)sizeof(typename F::E), CK::U, N, D, S, true, &hk)) return -6;
+    if (hk.lay.ps0 != CK::PS0 || hk.lay.vstride != CK::VSTRIDE || hk.lay.sc_v != CK::SC_V || hk.lay.sc_w != CK::SC_W ||
+        hk.lay.sc_scr != CK::SC_SCR || hk.lay.nscal != CK::NSCAL || hk.lay.nslots != CK::NSLOTS || hk.smem != CK::SMEM_BYTES)
+        return -7;
+    if (memcmp(&hk.tab, &h.tab, sizeof(h.tab)) != 0) return -8;       // same program: the ops do not name the W table
     return 0;
 }
 

@@ -65,7 +65,8 @@ def test_kernel_info_and_bad_shapes(lib):
     ki = binding.bg_kernel_info(0, 13, 5)                            # outside the compiled grid: run-time-n tiled kernel
     assert ki["specialised"] == 4 and ki["points_per_block"] == 32 and ki["threads_per_block"] == 256
     assert binding.bg_kernel_info(0, 16, 16)["points_per_block"] == 16   # two lanes per point: the 32-point tile is too large
-    assert binding.bg_kernel_info_problem(binding.problem(0, 13, 5, states=3))["specialised"] == 0   # general kernel
+    ki = binding.bg_kernel_info_problem(binding.problem(0, 13, 5, states=3))       # states / orderings on such a shape:
+    assert ki["specialised"] == 4 and ki["points_per_block"] == 32                  # the MULTI instantiation of bg_rt_kernel
     assert binding.bg_kernel_info(1, 6, 4)["specialised"] == 3       # cfg1: bg_reg_kernel ...
     pb = binding.problem(1, 6, 4, states=4)
     assert binding.bg_kernel_info_problem(pb)["specialised"] == 2    # ... but not with several state configurations
@@ -140,9 +141,14 @@ def test_default_kernels_do_not_spill(lib):
         stack, st, ld, regs = ents[name]
         assert (stack, st, ld) == (0, 0, 0), (name, ents[name])
         assert regs <= 255
-    # the run-time-n kernel over F_p (what shapes outside the compiled grid launch) may not spill more than a few words
-    worst = max((v[1] + v[2], k) for k, v in ents.items() if "bg_rt_kernel<bg::Fp31" in k or "bg_rt_kernel<bg::FpMont" in k)
-    assert worst[0] <= 64, worst
+    # the run-time-n kernel over F_p (what shapes outside the compiled grid launch) may spill a few words of set-up /
+    # loop state, not more (the complex128 instances at d >= 12 run at 255 registers and do spill: DESIGN.md §6.6)
+    rt = {k: v for k, v in ents.items() if "bg_rt_kernel<bg::Fp31" in k or "bg_rt_kernel<bg::FpMont" in k}
+    assert len(rt) >= 4 * 40
+    worst = max((v[1] + v[2], k) for k, v in rt.items() if k.endswith("false>"))
+    assert worst[0] <= 128, worst
+    worst = max((v[1] + v[2], k) for k, v in rt.items() if k.endswith("true>"))
+    assert worst[0] <= 256, worst
 
 
 def test_host_workspace_formula(lib):

@@ -334,6 +334,63 @@ def test_orderings_on_a_side_stream(bgl, oracle_mod):
     torch.cuda.synchronize()
 
 
+# ---- orderings x states on the run-time-n tiled kernel (MULTI instantiation of bg_rt_kernel) ------------------------
+RT_MULTI = [("fp31", 13, 5, 45, 3, 4, False),      # no compiled instance, one lane per point
+            ("fp31", 16, 4, 33, 2, 0, False),      # states only (the caller's order)
+            ("fp31", 16, 16, 20, 2, 3, False),     # two lanes per point (16-point tiles)
+            ("fp31", 11, 7, 40, 1, 5, False),      # orderings only
+            ("fp31", 8, 6, 70, 4, 6, True),        # compiled shapes, forced onto bg_rt_kernel
+            ("fp31", 4, 4, 70, 3, 2, True),
+            ("c128", 13, 4, 21, 2, 3, False), ("c128", 7, 5, 40, 2, 2, False), ("c128", 12, 6, 24, 2, 2, True)]
+
+
+@pytest.mark.parametrize("field,n,d,batch,S,K,force", RT_MULTI, ids=lambda v: str(v))
+def test_rt_kernel_orderings_and_states(bgl, oracle_mod, field, n, d, batch, S, K, force):
+    """S state configurations x K colour orderings per point on shapes without a compiled instance run the tiled
+    kernel (specialised == 4), not the one-thread-per-point fallback: bit-exact / rule R9 against the oracle, incl. a
+    singular point (status per momentum point, OR over the orderings) and a ragged last tile."""
+    import torch
+    from oracle import rule
+    f = bgl.FIELD_FP31 if field == "fp31" else bgl.FIELD_C128
+    perms = _perms(n, K, min(n, K)) if K else None
+    mom, pol, _ = inputs.make_state_inputs(field, n, d, batch, S, seed=29)
+    mom = mom.copy()
+    if field == "fp31":
+        mom[3, 1] = mom[3, 0]
+    if force:
+        bgl.bg_set_kernel_override("rt", 0)
+    try:
+        pb = bgl.problem(f, n, d, states=S, n_orderings=0 if perms is None else len(perms),
+                         orderings_ptr=None if perms is None else 4096)
+        ki = bgl.bg_kernel_info_problem(pb)
+        assert ki["specialised"] == 4, ki
+        status = torch.zeros(batch, dtype=torch.int32, device="cuda")
+        got = bgl.to_numpy(bgl.evaluate(bgl.to_device(mom), bgl.to_device(pol), orderings=perms, status=status))
+        torch.cuda.synchronize()
+    finally:
+        bgl.bg_set_kernel_override("default", 0)
+    ofield = oracle_mod.FP31 if field == "fp31" else oracle_mod.C128
+    if perms is None:
+        ref, rst = oracle_mod.evaluate(ofield, mom, pol, want_status=True, threads=8)
+    else:
+        ref = oracle_mod.orderings(ofield, mom, pol, perms, threads=8)
+        rst = np.zeros(batch, np.uint32)
+        for sg in perms:
+            rst |= oracle_mod.evaluate(ofield, mom[:, list(sg)], pol[..., list(sg), :], want_status=True, threads=8)[1]
+    assert got.shape == ref.shape
+    if field == "fp31":
+        assert np.array_equal(got, ref)
+        assert np.array_equal(status.cpu().numpy().astype(np.uint32), rst) and rst[3] == 1
+    else:
+        g2, pol_s = got.reshape(batch, -1, S), pol
+        for k in range(g2.shape[1]):
+            sg = list(perms[k]) if perms is not None else list(range(n))
+            for s_ in range(S):
+                ok, st = rule.check(g2[:, k, s_], rule.evaluate(np.ascontiguousarray(mom[:, sg]),
+                                                                np.ascontiguousarray(pol_s[:, s_][:, sg]), threads=8))
+                assert ok.all() and st["e_g"]["median"] < 1e-12, (k, s_, st)
+
+
 def test_orderings_entry_point_states_and_complex(bgl, oracle_mod):
     import torch
     from oracle import rule
